@@ -1,0 +1,119 @@
+/*
+ * pss.h — C ABI of the B200-native semi-implicit pseudo-spectral SPDE stepper.
+ *
+ * The library implements ONE thing: the per-timestep hot path of cuPSS (arXiv 2405.02410),
+ *     d phi = F[phi] dt + sqrt(2D) dW                                   (Eq. 1,  PAPER.md:13)
+ * on periodic 1D/2D/3D lattices, for a system of fields (Eq. 10-11)
+ *     dt phi_i = L_i phi_i + sum_j M_ij prod_k psi_k^{n_k} + noise,
+ * advanced with the semi-implicit update (Eq. 18)
+ *     phi_q <- (phi_q + dt N_q + nu_q) / (1 - dt L_q)
+ * following the six-step list of PAPER.md:128-135.  Every step of the path runs in hand-written
+ * sm_100a CUDA kernels; there is no CPU fallback: a call made without a usable CUDA device returns
+ * PSS_ECUDA.
+ *
+ * Conventions:
+ *   - axis 0 is x (fastest in user memory), then y, then z.  n[j], dx[j] for j >= ndim are ignored.
+ *   - q_j = 2 pi s(k_j) / (n_j dx_j), s(k) = k for k <= n/2 else k - n
+ *   - forward DFT unnormalised, inverse carries 1/N, N = prod n_j.
+ *   - user real data: element type = precision of the system, x fastest.
+ *   - half-spectrum (pss_get_field_fourier, pss_debug_noise): kx = 0..n0/2 fastest, then ky, then kz;
+ *     logical mode index m = (kz*n1 + ky)*(n0/2+1) + kx.  The library's internal layout differs.
+ *
+ * Ownership: the caller owns every buffer it passes and must keep the bound workspace alive until
+ * pss_destroy (or the next pss_bind).  The library owns the opaque handle and small host tables.
+ * Handles are not thread-safe.  No exceptions cross this boundary; there is no global state.
+ *
+ * Errors: every int-returning call gives 0 on success or a negative code:
+ *   PSS_EINVAL        bad id / negative power / NULL / aux used before defined / implicit term on aux
+ *   PSS_EUNSUPPORTED  n_j not a power of two, n_j < 8, n_j > 8192 (2D/3D axes must fit one CTA's
+ *                     shared memory; 1D n <= 8192), more than 3 dims, product of > 4 factors,
+ *                     table capacities exceeded (see PSS_MAX_*)
+ *   PSS_ESTATE        add_* after finalize; bind/step/get before finalize/bind
+ *   PSS_ECUDA         a CUDA call failed (sticky for the handle; text via pss_last_cuda_error)
+ */
+#ifndef PSS_H
+#define PSS_H
+#include <stddef.h>
+#include <stdint.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct pss_system pss_system;
+
+typedef enum { PSS_F32 = 0, PSS_F64 = 1 } pss_precision;
+enum { PSS_DEALIAS_PAPER = 0, PSS_DEALIAS_TWO_THIRDS = 1, PSS_DEALIAS_OFF = 2 };
+enum { PSS_OK = 0, PSS_EINVAL = -1, PSS_EUNSUPPORTED = -2, PSS_ESTATE = -3, PSS_ECUDA = -4 };
+
+/* capacities of the device-side term program */
+enum {
+  PSS_MAX_DYNAMIC = 4,   /* dynamic fields                                         */
+  PSS_MAX_FACTORS = 12,  /* distinct fields that appear in products of order >= 2  */
+  PSS_MAX_GROUPS = 8,    /* distinct (target field, outer operator) pairs          */
+  PSS_MAX_TERMS = 32,    /* product terms                                          */
+  PSS_MAX_LINOPS = 96    /* flattened operator monomials                           */
+};
+
+/* One operator monomial in Fourier space (keywords of PAPER.md:186-190):
+ *   coef * (q^2)^q2_pow * (1/|q|)^invq_pow * (i q_x)^iq_pow[0] (i q_y)^iq_pow[1] (i q_z)^iq_pow[2]
+ * (1/|q|)^p := 0 at q = 0; a monomial with an odd iq_pow[j] is 0 at the Nyquist index k_j = n_j/2. */
+typedef struct {
+  double coef;
+  int q2_pow;
+  int invq_pow;
+  int iq_pow[3];
+} pss_op;
+
+/* PAPER.md:141 (i): "evolver system(gpu, Nx, Ny, dx, dy, dt, output)".  n, dx: host arrays of 3. */
+int pss_create(pss_system **out, int ndim, const int64_t n[3], const double dx[3], double dt,
+               pss_precision prec, uint64_t seed);
+/* createField(name, dynamic).  *field_id receives the id (creation order). */
+int pss_add_field(pss_system *, const char *name, int dynamic, int *field_id);
+/* lhs term of "dt phi + lhs = rhs": L_q -= coef*Op(q).  Dynamic fields only. */
+int pss_add_linear(pss_system *, int field, const pss_op *op);
+/* intermediate field definition psi_q += coef*Op(q)*src_q; src is a dynamic
+ * field or an EARLIER aux field. */
+int pss_add_aux_def(pss_system *, int aux, const pss_op *op, int src);
+/* rhs term (Eq. 15): N_q += outer(q) * F[ prod_k factor_k(x) ].  nfactors == 1 is an
+ * explicit linear term evaluated in Fourier space (no transform, no mask).  factor_fields: host array. */
+int pss_add_term(pss_system *, int field, const pss_op *outer, int nfactors, const int *factor_fields);
+/* addNoise(field, "D*q^a"): <|nu_q|^2> = 2 D |q|^a dt N / dV. */
+int pss_set_noise(pss_system *, int field, double D, int q_power);
+/* de-aliasing rule: PAPER = cutoff 2/(n+1) per factor field, n its highest order. */
+int pss_set_dealias(pss_system *, int rule);
+/* validate, freeze the term list, plan the kernels; *workspace_bytes = device bytes pss_bind needs. */
+int pss_finalize(pss_system *, size_t *workspace_bytes);
+/* device_workspace: DEVICE pointer, 256-byte aligned, >= workspace_bytes, zero-initialised by this
+ * call.  cuda_stream: a cudaStream_t (NULL = default stream); all later work is issued on it. */
+int pss_bind(pss_system *, void *device_workspace, size_t bytes, void *cuda_stream);
+/* R2C of user real data (x fastest) into the state.  on_device: 1 = DEVICE pointer, 0 = HOST pointer
+ * (copied with cudaMemcpyAsync on the bound stream, then the stream is synchronised). */
+int pss_set_field(pss_system *, int field, const void *real_xfastest, int on_device);
+/* nsteps time steps, asynchronous on the bound stream.
+ * pss_step(a); pss_step(b) is bit-identical to pss_step(a+b). */
+int pss_step(pss_system *, int64_t nsteps);
+/* C2R of the (unmasked) state, including 1/N.  Host destination => stream synchronised on return. */
+int pss_get_field(pss_system *, int field, void *real_out, int on_device);
+/* the state in the logical half-spectrum layout, complex of the system precision. */
+int pss_get_field_fourier(pss_system *, int field, void *halfspectrum_out, int on_device);
+/* test hook for the noise stream (HOST pointers, either may be NULL): the 4 Philox4x32-10 words per
+ * logical mode m, and the unit Hermitian Gaussian z (complex of the system precision) the step uses. */
+int pss_debug_noise(pss_system *, int field, uint64_t step, uint32_t *bits4_per_mode, void *z_halfspectrum);
+/* measurement hook: nsteps (<= 4096) steps exactly as pss_step, with one CUDA-event pair around every
+ * kernel launch on the bound stream; synchronises.  Returns the mean device time per launch in ms and
+ * the launch count of each kernel family: [0] k_rows, [1] k_update, [2] k_mid (3D only).  Not for 1D. */
+int pss_profile_step(pss_system *, int64_t nsteps, double ms_per_launch[3], int64_t launches[3]);
+/* number of kernels this handle has launched so far (for bench.py's gpu_launches claim). */
+uint64_t pss_launch_count(const pss_system *);
+/* algorithmic bytes one step of this system must move: pruned != 0 gives B_alg,
+ * pruned == 0 gives B_model. */
+double pss_model_bytes_per_step(const pss_system *, int pruned);
+uint64_t pss_step_count(const pss_system *);
+const char *pss_strerror(int code);
+const char *pss_last_cuda_error(const pss_system *);
+void pss_destroy(pss_system *);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -1,0 +1,929 @@
+/*
+ * pss.cu — host side of libpss.so: the C ABI of include/pss.h, the term-list compiler
+ * (field system -> Program), the launch plan and the step loop.
+ *
+ * No CPU compute path exists here: every transform, product, operator, noise draw and update
+ * runs in the kernels of pss_kernels.cuh.  The host only validates, flattens the term list and
+ * launches.
+ */
+#include "../../include/pss.h"
+
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "pss_kernels.cuh"
+
+namespace {
+
+struct DefH { pss_op op; int src; };
+struct FieldH {
+  std::string name;
+  bool dynamic;
+  std::vector<DefH> defs;
+  std::vector<pss_op> lhs;
+  bool noisy;
+  double D;
+  int qpow;
+};
+struct TermH { int field; pss_op outer; std::vector<int> factors; };
+
+struct Plan {
+  Geo geo[3];
+  int upd_W, upd_threads; size_t upd_smem; int upd_blocks;
+  int row_Wc, row_threads; size_t row_smem; int row_blocks;
+  int mid_W, mid_threads; size_t mid_smem;
+  int one_threads; size_t one_smem; /* 1D */
+  int kx_keep_max;                  /* max over factors of the number of kept kx */
+};
+
+}  // namespace
+
+struct pss_system {
+  int ndim;
+  int64_t n[3];
+  double dx[3];
+  double dt;
+  int prec;
+  uint64_t seed;
+  int dealias;
+  bool finalized, bound, psix_valid;
+  uint64_t step;
+  std::vector<FieldH> fields;
+  std::vector<TermH> terms;
+  std::vector<int> dyn_slot;
+  Program P;
+  Plan plan;
+  size_t csize, rsize;
+  int64_t M, N; /* modes (half-spectrum), sites */
+  /* workspace carve-up (byte offsets) */
+  size_t off_state, off_psix, off_phat, off_scratch, off_ureal, off_tw[3], ws_need;
+  char *ws;
+  cudaStream_t stream;
+  std::string cuda_msg;
+  bool cuda_bad;
+  uint64_t launches;
+  /* pss_profile_step: one event pair per launch */
+  bool prof_on;
+  std::vector<cudaEvent_t> prof_ev;
+  std::vector<int> prof_kind;
+};
+
+namespace {
+
+bool is_pow2(int64_t v) { return v >= 1 && (v & (v - 1)) == 0; }
+int ilog2(int64_t v) { int l = 0; while ((1ll << l) < v) ++l; return l; }
+
+bool op_ok(const pss_system *s, const pss_op *op) {
+  if (!op) return false;
+  if (op->q2_pow < 0 || op->invq_pow < 0 || op->q2_pow > 24 || op->invq_pow > 24) return false;
+  for (int j = 0; j < 3; ++j) {
+    if (op->iq_pow[j] < 0 || op->iq_pow[j] > 24) return false;
+    if (j >= s->ndim && op->iq_pow[j] != 0) return false;
+  }
+  return std::isfinite(op->coef);
+}
+bool fid_ok(const pss_system *s, int f) { return f >= 0 && f < (int)s->fields.size(); }
+
+int cuda_fail(pss_system *s, cudaError_t e, const char *what) {
+  s->cuda_bad = true;
+  s->cuda_msg = std::string(what) + ": " + cudaGetErrorString(e);
+  return PSS_ECUDA;
+}
+#define CK(call)                                                   \
+  do {                                                             \
+    cudaError_t e_ = (call);                                       \
+    if (e_ != cudaSuccess) return cuda_fail(s, e_, #call);         \
+  } while (0)
+#define CKL(name)                                                  \
+  do {                                                             \
+    cudaError_t e_ = cudaGetLastError();                           \
+    if (e_ != cudaSuccess) return cuda_fail(s, e_, name);          \
+    s->launches += 1;                                              \
+  } while (0)
+
+/* ---- term-list compiler ---------------------------------------------------------------- */
+DOp link_op(const pss_system *s, const pss_op &op, int src_slot) {
+  DOp d;
+  std::memset(&d, 0, sizeof(d));
+  d.coef = op.coef;
+  d.m = (int8_t)op.q2_pow;
+  d.p = (int8_t)op.invq_pow;
+  uint8_t z = 0;
+  for (int j = 0; j < 3; ++j) {
+    d.a[j] = (int8_t)op.iq_pow[j];
+    if (j < s->ndim && (op.iq_pow[j] & 1) && s->n[j] > 1) z |= (uint8_t)(1u << j);
+  }
+  if (op.invq_pow > 0) z |= 8u;
+  d.zflags = z;
+  d.src = (int8_t)src_slot;
+  return d;
+}
+bool compose(const DOp &outer, const DOp &inner, DOp &r) {
+  r = inner;
+  r.coef = outer.coef * inner.coef;
+  const int m = outer.m + inner.m, p = outer.p + inner.p;
+  if (m > 100 || p > 100) return false;
+  r.m = (int8_t)m;
+  r.p = (int8_t)p;
+  for (int j = 0; j < 3; ++j) {
+    const int a = outer.a[j] + inner.a[j];
+    if (a > 100) return false;
+    r.a[j] = (int8_t)a;
+  }
+  r.zflags = outer.zflags | inner.zflags;
+  return true;
+}
+bool same_monomial(const DOp &a, const DOp &b) {
+  return a.m == b.m && a.p == b.p && a.a[0] == b.a[0] && a.a[1] == b.a[1] && a.a[2] == b.a[2] &&
+         a.zflags == b.zflags && a.src == b.src;
+}
+void push_merged(std::vector<DOp> &v, const DOp &d) {
+  for (DOp &e : v)
+    if (same_monomial(e, d)) { e.coef += d.coef; return; }
+  v.push_back(d);
+}
+
+/* field -> sum of monomials acting on dynamic fields (aux fields are linear in them) */
+bool flatten(const pss_system *s, std::vector<std::vector<DOp>> &flat) {
+  const int nf = (int)s->fields.size();
+  flat.assign(nf, std::vector<DOp>());
+  for (int f = 0; f < nf; ++f) {
+    const FieldH &F = s->fields[f];
+    if (F.dynamic) {
+      pss_op one = {1.0, 0, 0, {0, 0, 0}};
+      flat[f].push_back(link_op(s, one, s->dyn_slot[f]));
+      continue;
+    }
+    for (const DefH &d : F.defs) {
+      const DOp l = link_op(s, d.op, 0);
+      for (const DOp &e : flat[d.src]) {
+        DOp r;
+        if (!compose(l, e, r)) return false;
+        push_merged(flat[f], r);
+      }
+    }
+  }
+  return true;
+}
+
+int build_program(pss_system *s) {
+  Program &P = s->P;
+  std::memset(&P, 0, sizeof(P));
+  P.ndim = s->ndim;
+  double dV = 1.0;
+  for (int j = 0; j < 3; ++j) {
+    P.n[j] = (int32_t)s->n[j];
+    P.qs[j] = (j < s->ndim) ? 2.0 * 3.14159265358979323846 / ((double)s->n[j] * s->dx[j]) : 0.0;
+    if (j < s->ndim) dV *= s->dx[j];
+  }
+  P.nxh = (int32_t)(s->n[0] / 2 + 1);
+  P.dealias = s->dealias;
+  P.dt = s->dt;
+  P.invN = 1.0 / (double)s->N;
+  P.seed_lo = (uint32_t)(s->seed & 0xffffffffu);
+  P.seed_hi = (uint32_t)(s->seed >> 32);
+
+  const int nf = (int)s->fields.size();
+  s->dyn_slot.assign(nf, -1);
+  int ndyn = 0;
+  for (int f = 0; f < nf; ++f)
+    if (s->fields[f].dynamic) {
+      if (ndyn >= PSS_P_MAX_DYN) return PSS_EUNSUPPORTED;
+      s->dyn_slot[f] = ndyn++;
+    }
+  P.ndyn = ndyn;
+  std::vector<std::vector<DOp>> flat;
+  if (!flatten(s, flat)) return PSS_EUNSUPPORTED;
+
+  std::vector<DOp> lin;
+  /* factor fields: appear in a product of order >= 2 */
+  std::vector<int> fac_slot(nf, -1);
+  int nfac = 0;
+  for (int f = 0; f < nf; ++f) {
+    int order = 0;
+    for (const TermH &t : s->terms) {
+      if (t.factors.size() < 2) continue;
+      for (int g : t.factors)
+        if (g == f && (int)t.factors.size() > order) order = (int)t.factors.size();
+    }
+    if (order < 2) continue;
+    if (nfac >= PSS_P_MAX_FAC) return PSS_EUNSUPPORTED;
+    DFactor &F = P.fac[nfac];
+    F.lin_beg = (int16_t)lin.size();
+    for (const DOp &e : flat[f]) lin.push_back(e);
+    F.lin_end = (int16_t)lin.size();
+    F.order = (int16_t)order;
+    fac_slot[f] = nfac++;
+  }
+  P.nfac = nfac;
+  /* groups of product terms: same target, same outer monomial (coef moves into the term) */
+  int ngrp = 0, nterm = 0;
+  std::vector<std::vector<DTerm>> gterms;
+  for (const TermH &t : s->terms) {
+    if (t.factors.size() < 2) continue;
+    DOp o = link_op(s, t.outer, s->dyn_slot[t.field]);
+    o.coef = 1.0;
+    int g = -1;
+    for (int i = 0; i < ngrp; ++i)
+      if (P.grp[i].target == s->dyn_slot[t.field] && same_monomial(P.grp[i].outer, o)) g = i;
+    if (g < 0) {
+      if (ngrp >= PSS_P_MAX_GRP) return PSS_EUNSUPPORTED;
+      g = ngrp++;
+      P.grp[g].outer = o;
+      P.grp[g].target = (int16_t)s->dyn_slot[t.field];
+      gterms.push_back(std::vector<DTerm>());
+    }
+    DTerm dt;
+    std::memset(&dt, 0, sizeof(dt));
+    dt.coef = t.outer.coef;
+    dt.nf = (int8_t)t.factors.size();
+    for (size_t i = 0; i < t.factors.size(); ++i) dt.f[i] = (int8_t)fac_slot[t.factors[i]];
+    gterms[g].push_back(dt);
+    ++nterm;
+  }
+  if (nterm > PSS_P_MAX_TERM) return PSS_EUNSUPPORTED;
+  int tpos = 0;
+  for (int g = 0; g < ngrp; ++g) {
+    P.grp[g].term_beg = (int16_t)tpos;
+    for (const DTerm &dt : gterms[g]) P.term[tpos++] = dt;
+    P.grp[g].term_end = (int16_t)tpos;
+  }
+  P.ngrp = ngrp;
+  P.nterm = nterm;
+  /* per dynamic field: lhs, explicit linear terms, noise */
+  for (int f = 0; f < nf; ++f) {
+    if (!s->fields[f].dynamic) continue;
+    const FieldH &F = s->fields[f];
+    DDyn &d = P.dyn[s->dyn_slot[f]];
+    d.field_id = f;
+    d.lhs_beg = (int16_t)lin.size();
+    {
+      std::vector<DOp> tmp;
+      for (const pss_op &op : F.lhs) push_merged(tmp, link_op(s, op, s->dyn_slot[f]));
+      for (const DOp &e : tmp) lin.push_back(e);
+    }
+    d.lhs_end = (int16_t)lin.size();
+    d.lin_beg = (int16_t)lin.size();
+    {
+      std::vector<DOp> tmp;
+      for (const TermH &t : s->terms) {
+        if (t.field != f || t.factors.size() != 1) continue;
+        const DOp l = link_op(s, t.outer, 0);
+        for (const DOp &e : flat[t.factors[0]]) {
+          DOp r;
+          if (!compose(l, e, r)) return PSS_EUNSUPPORTED;
+          push_merged(tmp, r);
+        }
+      }
+      for (const DOp &e : tmp) lin.push_back(e);
+    }
+    d.lin_end = (int16_t)lin.size();
+    d.noisy = F.noisy ? 1 : 0;
+    d.noise_qpow = (int16_t)F.qpow;
+    d.noise_c = 2.0 * F.D * s->dt * (double)s->N / dV;
+  }
+  if (lin.size() > PSS_P_MAX_LIN) return PSS_EUNSUPPORTED;
+  for (size_t i = 0; i < lin.size(); ++i) P.lin[i] = lin[i];
+  P.nlin = (int32_t)lin.size();
+  return PSS_OK;
+}
+
+/* ---- launch plan ----------------------------------------------------------------------- */
+Geo make_geo(int64_t n) {
+  Geo g;
+  std::memset(&g, 0, sizeof(g));
+  g.n = (int32_t)n;
+  const int lg = ilog2(n);
+  const int np = (lg + 3) / 4;
+  g.nr = np;
+  for (int q = 0; q < np; ++q) g.lg[q] = lg / np + (q < lg % np ? 1 : 0);
+  return g;
+}
+
+int env_int(const char *name, int dflt) {
+  const char *v = std::getenv(name);
+  return (v && *v) ? std::atoi(v) : dflt;
+}
+
+const size_t SMEM_MAX = 227 * 1024;
+const size_t SMEM_SOFT = 100 * 1024; /* leaves room for two CTAs per SM */
+
+int round_threads(long long work) {
+  long long t = ((work + 31) / 32) * 32;
+  if (t < 64) t = 64;
+  if (t > 256) t = 256;
+  return (int)t;
+}
+
+int make_plan(pss_system *s) {
+  Plan &pl = s->plan;
+  std::memset(&pl, 0, sizeof(pl));
+  const Program &P = s->P;
+  for (int j = 0; j < 3; ++j) pl.geo[j] = make_geo(s->n[j]);
+  const size_t cs = s->csize;
+  const int nxh = P.nxh;
+  pl.kx_keep_max = 0;
+  for (int f = 0; f < P.nfac; ++f) {
+    int cut = nxh;
+    if (P.dealias != PSS_DEALIAS_OFF) {
+      const int nn = (P.dealias == PSS_DEALIAS_TWO_THIRDS ? 2 : P.fac[f].order) + 1;
+      cut = (int)((s->n[0] + nn - 1) / nn);
+      if (cut > nxh) cut = nxh;
+    }
+    if (cut > pl.kx_keep_max) pl.kx_keep_max = cut;
+  }
+  if (s->ndim == 1) {
+    const size_t bufs = (size_t)(P.nfac + P.ngrp);
+    pl.one_smem = bufs * (size_t)s->n[0] * cs;
+    if (pl.one_smem > SMEM_MAX) return PSS_EUNSUPPORTED;
+    if (pl.one_smem < 16) pl.one_smem = 16;
+    pl.one_threads = round_threads(s->n[0] / 4);
+    return PSS_OK;
+  }
+  /* k_update: W contiguous last-axis lines per CTA */
+  {
+    const int64_t n = s->n[s->ndim - 1];
+    const int64_t nlines = (s->ndim == 3) ? (int64_t)nxh * s->n[1] : nxh;
+    const int nb0 = P.ngrp > P.ndyn ? P.ngrp : P.ndyn;
+    const size_t per = (size_t)(nb0 + (P.nfac > 1 ? 1 : 0)) * (size_t)n * cs;
+    if (per > SMEM_MAX) return PSS_EUNSUPPORTED;
+    int W = 1;
+    for (int cand = 8; cand >= 1; cand >>= 1) {
+      if (per * cand > SMEM_SOFT && cand > 1) continue;
+      if ((nlines + cand - 1) / cand < 2 * 148 && cand > 1) continue;
+      W = cand;
+      break;
+    }
+    W = env_int("PSS_UPD_W", W);
+    if (W < 1) W = 1;
+    while (W > 1 && per * W > SMEM_MAX) W >>= 1;
+    pl.upd_W = W;
+    pl.upd_smem = per * W;
+    pl.upd_blocks = (int)((nlines + W - 1) / W);
+    pl.upd_threads = env_int("PSS_UPD_T", round_threads((n / 8) * W * (P.ngrp > 0 ? P.ngrp : 1)));
+  }
+  /* k_rows: Wc pairs of rows per CTA (2*Wc contiguous rows of every kx) */
+  if (P.ngrp > 0) {
+    const int64_t nx = s->n[0];
+    const int64_t R = s->N / nx;
+    const size_t per = (size_t)(P.nfac + (P.ngrp > 1 ? 1 : 0)) * (size_t)nx * cs;
+    if (per > SMEM_MAX) return PSS_EUNSUPPORTED;
+    const int wc_sector = (cs == 8) ? 2 : 1; /* 2*Wc complex = one 32-byte sector */
+    int Wc = 1;
+    for (int cand = 8; cand >= 1; cand >>= 1) {
+      if (2 * cand > R) continue;
+      if (per * cand > SMEM_SOFT && cand > 1) continue;
+      if (R / (2 * cand) < 2 * 148 && cand > wc_sector) continue;
+      Wc = cand;
+      break;
+    }
+    Wc = env_int("PSS_ROW_WC", Wc);
+    if (Wc < 1) Wc = 1;
+    while (Wc > 1 && (per * Wc > SMEM_MAX || 2 * Wc > R || R % (2 * Wc) != 0)) Wc >>= 1;
+    pl.row_Wc = Wc;
+    pl.row_smem = per * Wc;
+    pl.row_blocks = (int)(R / (2 * Wc));
+    pl.row_threads = env_int("PSS_ROW_T", round_threads((nx / 8) * Wc * (P.nfac > 0 ? P.nfac : 1)));
+  }
+  if (s->ndim == 3) {
+    int W = (int)(128 / cs);
+    if (W > s->n[2]) W = (int)s->n[2];
+    while ((size_t)W * s->n[1] * cs > SMEM_MAX && W > 1) W >>= 1;
+    if ((size_t)W * s->n[1] * cs > SMEM_MAX) return PSS_EUNSUPPORTED;
+    pl.mid_W = W;
+    pl.mid_smem = (size_t)W * s->n[1] * cs;
+    pl.mid_threads = round_threads((s->n[1] / 8) * W);
+  }
+  return PSS_OK;
+}
+
+size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+void carve_workspace(pss_system *s) {
+  const Program &P = s->P;
+  size_t off = 0;
+  const size_t arr = align_up((size_t)s->M * s->csize, 256);
+  s->off_state = off; off += arr * (size_t)P.ndyn;
+  s->off_psix = off;  off += arr * (size_t)(P.nfac > 0 ? P.nfac : 0);
+  s->off_phat = off;  off += arr * (size_t)(P.ngrp > 0 ? P.ngrp : 0);
+  s->off_scratch = off; off += arr;
+  s->off_ureal = off; off += align_up((size_t)s->N * s->rsize, 256);
+  for (int j = 0; j < 3; ++j) { s->off_tw[j] = off; off += align_up((size_t)s->n[j] * s->csize, 256); }
+  s->ws_need = off;
+}
+
+template <typename T> typename cplx_of<T>::type *carr(pss_system *s, size_t off, int idx) {
+  const size_t arr = align_up((size_t)s->M * s->csize, 256);
+  return reinterpret_cast<typename cplx_of<T>::type *>(s->ws + off + arr * (size_t)idx);
+}
+/* NOTE: arrays of one kind are spaced by the ALIGNED size; kernels take M_stride = arr / csize */
+long long arr_stride(const pss_system *s) { return (long long)(align_up((size_t)s->M * s->csize, 256) / s->csize); }
+
+template <typename T> const typename cplx_of<T>::type *twp(pss_system *s, int axis) {
+  return reinterpret_cast<const typename cplx_of<T>::type *>(s->ws + s->off_tw[axis]);
+}
+
+template <typename T> int set_attrs(pss_system *s) {
+  CK(cudaFuncSetAttribute(k_update<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_MAX));
+  CK(cudaFuncSetAttribute(k_rows<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_MAX));
+  CK(cudaFuncSetAttribute(k_mid<-1, T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_MAX));
+  CK(cudaFuncSetAttribute(k_mid<+1, T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_MAX));
+  CK(cudaFuncSetAttribute(k_last<-1, T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_MAX));
+  CK(cudaFuncSetAttribute(k_last<+1, T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_MAX));
+  CK(cudaFuncSetAttribute(k_user_x<-1, T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_MAX));
+  CK(cudaFuncSetAttribute(k_user_x<+1, T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_MAX));
+  CK(cudaFuncSetAttribute(k_step1d<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_MAX));
+  return PSS_OK;
+}
+
+template <typename T> int upload_twiddles(pss_system *s) {
+  typedef typename cplx_of<T>::type C;
+  for (int j = 0; j < s->ndim; ++j) {
+    std::vector<C> tw((size_t)s->n[j]);
+    const long double PI_L = 3.14159265358979323846264338327950288L;
+    for (int64_t i = 0; i < s->n[j]; ++i) {
+      const long double a = 2.0L * PI_L * (long double)i / (long double)s->n[j];
+      tw[(size_t)i].x = (T)cosl(a);
+      tw[(size_t)i].y = (T)(-sinl(a));
+    }
+    CK(cudaMemcpyAsync(s->ws + s->off_tw[j], tw.data(), tw.size() * sizeof(C), cudaMemcpyHostToDevice, s->stream));
+    CK(cudaStreamSynchronize(s->stream)); /* tw is a stack-lifetime host buffer */
+  }
+  return PSS_OK;
+}
+
+/* ---- launches -------------------------------------------------------------------------- */
+enum { KIND_ROWS = 0, KIND_UPDATE = 1, KIND_MID = 2 };
+void prof_mark(pss_system *s, int kind, bool begin) {
+  if (!s->prof_on) return;
+  cudaEvent_t e;
+  if (cudaEventCreate(&e) != cudaSuccess) return;
+  cudaEventRecord(e, s->stream);
+  s->prof_ev.push_back(e);
+  if (begin) s->prof_kind.push_back(kind);
+}
+
+template <typename T> int launch_mid(pss_system *s, int sgn, size_t off, int nbatch, int kx_count, bool factor_mask = false) {
+  MidArgs<T> a;
+  std::memset(&a, 0, sizeof(a));
+  a.nx = (int)s->n[0];
+  if (factor_mask && s->P.dealias != PSS_DEALIAS_OFF)
+    for (int f = 0; f < nbatch; ++f) a.nn[f] = (s->P.dealias == PSS_DEALIAS_TWO_THIRDS ? 2 : s->P.fac[f].order) + 1;
+  a.arr = carr<T>(s, off, 0);
+  a.tw = twp<T>(s, 1);
+  a.M = arr_stride(s);
+  a.ny = (int)s->n[1];
+  a.nz = (int)s->n[2];
+  a.W = s->plan.mid_W;
+  a.kx_count = kx_count;
+  a.geo = s->plan.geo[1];
+  dim3 grid((unsigned)(s->n[2] / s->plan.mid_W), (unsigned)kx_count, (unsigned)nbatch);
+  prof_mark(s, KIND_MID, true);
+  if (sgn < 0) k_mid<-1, T><<<grid, s->plan.mid_threads, s->plan.mid_smem, s->stream>>>(a);
+  else k_mid<+1, T><<<grid, s->plan.mid_threads, s->plan.mid_smem, s->stream>>>(a);
+  prof_mark(s, KIND_MID, false);
+  CKL("k_mid");
+  return PSS_OK;
+}
+
+template <typename T> int launch_update(pss_system *s, int prologue, uint64_t step) {
+  const Program &P = s->P;
+  UpdArgs<T> a;
+  a.state = carr<T>(s, s->off_state, 0);
+  a.psix = carr<T>(s, s->off_psix, 0);
+  a.phat = carr<T>(s, s->off_phat, 0);
+  a.tw = twp<T>(s, s->ndim - 1);
+  a.M = arr_stride(s);
+  a.n = (int)s->n[s->ndim - 1];
+  a.nlines = (s->ndim == 3) ? (int)(P.nxh * s->n[1]) : P.nxh;
+  a.W = s->plan.upd_W;
+  a.prologue = prologue;
+  a.step = step;
+  a.geo = s->plan.geo[s->ndim - 1];
+  prof_mark(s, KIND_UPDATE, true);
+  k_update<T><<<s->plan.upd_blocks, s->plan.upd_threads, s->plan.upd_smem, s->stream>>>(P, a);
+  prof_mark(s, KIND_UPDATE, false);
+  CKL("k_update");
+  if (s->ndim == 3 && P.nfac > 0) return launch_mid<T>(s, +1, s->off_psix, P.nfac, s->plan.kx_keep_max, true);
+  return PSS_OK;
+}
+
+template <typename T> int launch_rows(pss_system *s) {
+  const Program &P = s->P;
+  RowArgs<T> a;
+  a.psix = carr<T>(s, s->off_psix, 0);
+  a.phat = carr<T>(s, s->off_phat, 0);
+  a.tw = twp<T>(s, 0);
+  a.M = arr_stride(s);
+  a.R = s->N / s->n[0];
+  a.nx = (int)s->n[0];
+  a.Wc = s->plan.row_Wc;
+  a.geo = s->plan.geo[0];
+  prof_mark(s, KIND_ROWS, true);
+  k_rows<T><<<s->plan.row_blocks, s->plan.row_threads, s->plan.row_smem, s->stream>>>(P, a);
+  prof_mark(s, KIND_ROWS, false);
+  CKL("k_rows");
+  if (s->ndim == 3) return launch_mid<T>(s, -1, s->off_phat, P.ngrp, P.nxh);
+  return PSS_OK;
+}
+
+template <typename T> int do_steps(pss_system *s, int64_t nsteps) {
+  const Program &P = s->P;
+  if (nsteps == 0) return PSS_OK;
+  if (s->ndim == 1) {
+    Step1dArgs<T> a;
+    a.state = carr<T>(s, s->off_state, 0);
+    a.tw = twp<T>(s, 0);
+    a.M = arr_stride(s);
+    a.nx = (int)s->n[0];
+    a.nsteps = nsteps;
+    a.step0 = s->step;
+    a.geo = s->plan.geo[0];
+    k_step1d<T><<<1, s->plan.one_threads, s->plan.one_smem, s->stream>>>(P, a);
+    CKL("k_step1d");
+    s->step += (uint64_t)nsteps;
+    return PSS_OK;
+  }
+  int rc;
+  if (P.nfac > 0 && !s->psix_valid) {
+    if ((rc = launch_update<T>(s, 1, s->step)) != PSS_OK) return rc;
+    s->psix_valid = true;
+  }
+  for (int64_t i = 0; i < nsteps; ++i) {
+    if (P.ngrp > 0 && (rc = launch_rows<T>(s)) != PSS_OK) return rc;
+    if ((rc = launch_update<T>(s, 0, s->step)) != PSS_OK) return rc;
+    s->step += 1;
+  }
+  return PSS_OK;
+}
+
+template <typename T> int do_set_field(pss_system *s, int slot, const void *src, int on_device) {
+  const T *real = (const T *)src;
+  if (!on_device) {
+    CK(cudaMemcpyAsync(s->ws + s->off_ureal, src, (size_t)s->N * sizeof(T), cudaMemcpyHostToDevice, s->stream));
+    real = (const T *)(s->ws + s->off_ureal);
+  }
+  UserArgs<T> a;
+  a.real = const_cast<T *>(real);
+  a.arr = carr<T>(s, s->off_state, slot);
+  a.tw = twp<T>(s, 0);
+  a.nx = (int)s->n[0];
+  a.ny = (int)s->n[1];
+  a.nz = (int)s->n[2];
+  a.single = (s->ndim == 1) ? 1 : 0;
+  a.scale = 1.0;
+  a.geo = s->plan.geo[0];
+  const int64_t R = s->N / s->n[0];
+  const unsigned blocks = (unsigned)(a.single ? R : R / 2);
+  k_user_x<-1, T><<<blocks, round_threads(s->n[0] / 4), (size_t)s->n[0] * sizeof(typename cplx_of<T>::type), s->stream>>>(a);
+  CKL("k_user_x");
+  if (s->ndim == 3) {
+    const int rc = launch_mid<T>(s, -1, s->off_state + (size_t)slot * (size_t)arr_stride(s) * s->csize, 1, s->P.nxh);
+    if (rc != PSS_OK) return rc;
+  }
+  if (s->ndim >= 2) {
+    LastArgs<T> l;
+    l.arr = carr<T>(s, s->off_state, slot);
+    l.tw = twp<T>(s, s->ndim - 1);
+    l.n = (int)s->n[s->ndim - 1];
+    l.nlines = (int)(s->M / l.n);
+    l.geo = s->plan.geo[s->ndim - 1];
+    k_last<-1, T><<<l.nlines, round_threads(l.n / 4), (size_t)l.n * sizeof(typename cplx_of<T>::type), s->stream>>>(l);
+    CKL("k_last");
+  }
+  s->psix_valid = false;
+  if (!on_device) CK(cudaStreamSynchronize(s->stream));
+  return PSS_OK;
+}
+
+template <typename T> int do_get_field(pss_system *s, int slot, void *dst, int on_device) {
+  typedef typename cplx_of<T>::type C;
+  CK(cudaMemcpyAsync(s->ws + s->off_scratch, carr<T>(s, s->off_state, slot), (size_t)s->M * sizeof(C),
+                     cudaMemcpyDeviceToDevice, s->stream));
+  if (s->ndim >= 2) {
+    LastArgs<T> l;
+    l.arr = carr<T>(s, s->off_scratch, 0);
+    l.tw = twp<T>(s, s->ndim - 1);
+    l.n = (int)s->n[s->ndim - 1];
+    l.nlines = (int)(s->M / l.n);
+    l.geo = s->plan.geo[s->ndim - 1];
+    k_last<+1, T><<<l.nlines, round_threads(l.n / 4), (size_t)l.n * sizeof(C), s->stream>>>(l);
+    CKL("k_last");
+  }
+  if (s->ndim == 3) {
+    const int rc = launch_mid<T>(s, +1, s->off_scratch, 1, s->P.nxh);
+    if (rc != PSS_OK) return rc;
+  }
+  UserArgs<T> a;
+  a.real = on_device ? (T *)dst : (T *)(s->ws + s->off_ureal);
+  a.arr = carr<T>(s, s->off_scratch, 0);
+  a.tw = twp<T>(s, 0);
+  a.nx = (int)s->n[0];
+  a.ny = (int)s->n[1];
+  a.nz = (int)s->n[2];
+  a.single = (s->ndim == 1) ? 1 : 0;
+  a.scale = 1.0 / (double)s->N;
+  a.geo = s->plan.geo[0];
+  const int64_t R = s->N / s->n[0];
+  const unsigned blocks = (unsigned)(a.single ? R : R / 2);
+  k_user_x<+1, T><<<blocks, round_threads(s->n[0] / 4), (size_t)s->n[0] * sizeof(C), s->stream>>>(a);
+  CKL("k_user_x");
+  if (!on_device) {
+    CK(cudaMemcpyAsync(dst, s->ws + s->off_ureal, (size_t)s->N * sizeof(T), cudaMemcpyDeviceToHost, s->stream));
+    CK(cudaStreamSynchronize(s->stream));
+  }
+  return PSS_OK;
+}
+
+template <typename T> int do_get_fourier(pss_system *s, int slot, void *dst, int on_device) {
+  typedef typename cplx_of<T>::type C;
+  C *out = on_device ? (C *)dst : carr<T>(s, s->off_scratch, 0);
+  k_to_logical<T><<<592, 256, 0, s->stream>>>(carr<T>(s, s->off_state, slot), out, s->P.nxh, (int)s->n[1], (int)s->n[2]);
+  CKL("k_to_logical");
+  if (!on_device) {
+    CK(cudaMemcpyAsync(dst, out, (size_t)s->M * sizeof(C), cudaMemcpyDeviceToHost, s->stream));
+    CK(cudaStreamSynchronize(s->stream));
+  }
+  return PSS_OK;
+}
+
+template <typename T> int do_debug_noise(pss_system *s, int field, uint64_t step, uint32_t *bits, void *z) {
+  typedef typename cplx_of<T>::type C;
+  uint32_t *dbits = nullptr;
+  C *dz = nullptr;
+  if (bits) CK(cudaMalloc(&dbits, (size_t)s->M * 4 * sizeof(uint32_t)));
+  if (z) CK(cudaMalloc(&dz, (size_t)s->M * sizeof(C)));
+  k_debug_noise<T><<<592, 256, 0, s->stream>>>(s->P, field, step, dbits, dz);
+  CKL("k_debug_noise");
+  if (bits) CK(cudaMemcpyAsync(bits, dbits, (size_t)s->M * 4 * sizeof(uint32_t), cudaMemcpyDeviceToHost, s->stream));
+  if (z) CK(cudaMemcpyAsync(z, dz, (size_t)s->M * sizeof(C), cudaMemcpyDeviceToHost, s->stream));
+  CK(cudaStreamSynchronize(s->stream));
+  if (dbits) cudaFree(dbits);
+  if (dz) cudaFree(dz);
+  return PSS_OK;
+}
+
+}  // namespace
+
+/* ---- C ABI ----------------------------------------------------------------------------- */
+extern "C" {
+
+int pss_create(pss_system **out, int ndim, const int64_t n[3], const double dx[3], double dt,
+               pss_precision prec, uint64_t seed) {
+  if (!out || !n || !dx) return PSS_EINVAL;
+  *out = nullptr;
+  if (ndim < 1) return PSS_EINVAL;
+  if (ndim > 3) return PSS_EUNSUPPORTED;
+  if (prec != PSS_F32 && prec != PSS_F64) return PSS_EINVAL;
+  if (!(dt > 0.0) || !std::isfinite(dt)) return PSS_EINVAL;
+  for (int j = 0; j < ndim; ++j) {
+    if (n[j] < 1 || !(dx[j] > 0.0) || !std::isfinite(dx[j])) return PSS_EINVAL;
+    if (!is_pow2(n[j]) || n[j] < 8 || n[j] > 8192) return PSS_EUNSUPPORTED; /* A17 */
+  }
+  pss_system *s = new pss_system();
+  s->ndim = ndim;
+  for (int j = 0; j < 3; ++j) { s->n[j] = j < ndim ? n[j] : 1; s->dx[j] = j < ndim ? dx[j] : 1.0; }
+  s->dt = dt;
+  s->prec = (int)prec;
+  s->seed = seed;
+  s->dealias = PSS_DEALIAS_PAPER;
+  s->finalized = s->bound = s->psix_valid = false;
+  s->step = 0;
+  s->csize = prec == PSS_F32 ? 8 : 16;
+  s->rsize = prec == PSS_F32 ? 4 : 8;
+  s->N = s->n[0] * s->n[1] * s->n[2];
+  s->M = (s->n[0] / 2 + 1) * s->n[1] * s->n[2];
+  s->ws = nullptr;
+  s->stream = nullptr;
+  s->cuda_bad = false;
+  s->launches = 0;
+  s->prof_on = false;
+  *out = s;
+  return PSS_OK;
+}
+
+int pss_add_field(pss_system *s, const char *name, int dynamic, int *field_id) {
+  if (!s || !name) return PSS_EINVAL;
+  if (s->finalized) return PSS_ESTATE;
+  if (s->fields.size() >= 64) return PSS_EUNSUPPORTED;
+  for (const FieldH &f : s->fields) if (f.name == name) return PSS_EINVAL;
+  FieldH f;
+  f.name = name; f.dynamic = dynamic != 0; f.noisy = false; f.D = 0; f.qpow = 0;
+  s->fields.push_back(f);
+  if (field_id) *field_id = (int)s->fields.size() - 1;
+  return PSS_OK;
+}
+
+int pss_add_linear(pss_system *s, int field, const pss_op *op) {
+  if (!s) return PSS_EINVAL;
+  if (s->finalized) return PSS_ESTATE;
+  if (!fid_ok(s, field) || !op_ok(s, op)) return PSS_EINVAL;
+  if (!s->fields[field].dynamic) return PSS_EINVAL;
+  s->fields[field].lhs.push_back(*op);
+  return PSS_OK;
+}
+
+int pss_add_aux_def(pss_system *s, int aux, const pss_op *op, int src) {
+  if (!s) return PSS_EINVAL;
+  if (s->finalized) return PSS_ESTATE;
+  if (!fid_ok(s, aux) || !fid_ok(s, src) || !op_ok(s, op)) return PSS_EINVAL;
+  if (s->fields[aux].dynamic) return PSS_EINVAL;
+  if (!s->fields[src].dynamic && src >= aux) return PSS_EINVAL; /* A12 */
+  DefH d; d.op = *op; d.src = src;
+  s->fields[aux].defs.push_back(d);
+  return PSS_OK;
+}
+
+int pss_add_term(pss_system *s, int field, const pss_op *outer, int nfactors, const int *factor_fields) {
+  if (!s) return PSS_EINVAL;
+  if (s->finalized) return PSS_ESTATE;
+  if (!fid_ok(s, field) || !op_ok(s, outer) || !factor_fields) return PSS_EINVAL;
+  if (!s->fields[field].dynamic) return PSS_EINVAL;
+  if (nfactors < 1) return PSS_EINVAL;
+  if (nfactors > 4) return PSS_EUNSUPPORTED;
+  TermH t; t.field = field; t.outer = *outer;
+  for (int i = 0; i < nfactors; ++i) {
+    if (!fid_ok(s, factor_fields[i])) return PSS_EINVAL;
+    t.factors.push_back(factor_fields[i]);
+  }
+  s->terms.push_back(t);
+  return PSS_OK;
+}
+
+int pss_set_noise(pss_system *s, int field, double D, int q_power) {
+  if (!s) return PSS_EINVAL;
+  if (s->finalized) return PSS_ESTATE;
+  if (!fid_ok(s, field) || !s->fields[field].dynamic) return PSS_EINVAL;
+  if (!(D >= 0.0) || !std::isfinite(D)) return PSS_EINVAL;
+  if (q_power < -8 || q_power > 8) return PSS_EINVAL;
+  FieldH &f = s->fields[field];
+  f.noisy = D > 0.0; f.D = D; f.qpow = q_power;
+  return PSS_OK;
+}
+
+int pss_set_dealias(pss_system *s, int rule) {
+  if (!s) return PSS_EINVAL;
+  if (s->finalized) return PSS_ESTATE;
+  if (rule < PSS_DEALIAS_PAPER || rule > PSS_DEALIAS_OFF) return PSS_EINVAL;
+  s->dealias = rule;
+  return PSS_OK;
+}
+
+int pss_finalize(pss_system *s, size_t *workspace_bytes) {
+  if (!s) return PSS_EINVAL;
+  if (s->finalized) return PSS_ESTATE;
+  int ndyn = 0;
+  for (const FieldH &f : s->fields) ndyn += f.dynamic ? 1 : 0;
+  if (ndyn == 0) return PSS_EINVAL;
+  for (const FieldH &f : s->fields)
+    if (!f.dynamic && f.defs.empty()) return PSS_EINVAL;
+  if (s->fields.size() > 0xffff) return PSS_EUNSUPPORTED;
+  int rc = build_program(s);
+  if (rc != PSS_OK) return rc;
+  rc = make_plan(s);
+  if (rc != PSS_OK) return rc;
+  carve_workspace(s);
+  s->finalized = true;
+  if (workspace_bytes) *workspace_bytes = s->ws_need;
+  return PSS_OK;
+}
+
+int pss_bind(pss_system *s, void *device_workspace, size_t bytes, void *cuda_stream) {
+  if (!s || !device_workspace) return PSS_EINVAL;
+  if (!s->finalized) return PSS_ESTATE;
+  if (bytes < s->ws_need || ((uintptr_t)device_workspace & 255u)) return PSS_EINVAL;
+  int ndev = 0;
+  CK(cudaGetDeviceCount(&ndev));
+  if (ndev < 1) return cuda_fail(s, cudaErrorNoDevice, "pss_bind");
+  s->ws = (char *)device_workspace;
+  s->stream = (cudaStream_t)cuda_stream;
+  CK(cudaMemsetAsync(s->ws, 0, s->ws_need, s->stream));
+  int rc = (s->prec == PSS_F32) ? set_attrs<float>(s) : set_attrs<double>(s);
+  if (rc != PSS_OK) return rc;
+  rc = (s->prec == PSS_F32) ? upload_twiddles<float>(s) : upload_twiddles<double>(s);
+  if (rc != PSS_OK) return rc;
+  s->bound = true;
+  s->psix_valid = false;
+  return PSS_OK;
+}
+
+int pss_set_field(pss_system *s, int field, const void *real_xfastest, int on_device) {
+  if (!s || !real_xfastest) return PSS_EINVAL;
+  if (!s->finalized || !s->bound) return PSS_ESTATE;
+  if (s->cuda_bad) return PSS_ECUDA;
+  if (!fid_ok(s, field) || !s->fields[field].dynamic) return PSS_EINVAL;
+  const int slot = s->dyn_slot[field];
+  return (s->prec == PSS_F32) ? do_set_field<float>(s, slot, real_xfastest, on_device)
+                              : do_set_field<double>(s, slot, real_xfastest, on_device);
+}
+
+int pss_step(pss_system *s, int64_t nsteps) {
+  if (!s || nsteps < 0) return PSS_EINVAL;
+  if (!s->finalized || !s->bound) return PSS_ESTATE;
+  if (s->cuda_bad) return PSS_ECUDA;
+  return (s->prec == PSS_F32) ? do_steps<float>(s, nsteps) : do_steps<double>(s, nsteps);
+}
+
+int pss_get_field(pss_system *s, int field, void *real_out, int on_device) {
+  if (!s || !real_out) return PSS_EINVAL;
+  if (!s->finalized || !s->bound) return PSS_ESTATE;
+  if (s->cuda_bad) return PSS_ECUDA;
+  if (!fid_ok(s, field) || !s->fields[field].dynamic) return PSS_EINVAL;
+  const int slot = s->dyn_slot[field];
+  return (s->prec == PSS_F32) ? do_get_field<float>(s, slot, real_out, on_device)
+                              : do_get_field<double>(s, slot, real_out, on_device);
+}
+
+int pss_get_field_fourier(pss_system *s, int field, void *out, int on_device) {
+  if (!s || !out) return PSS_EINVAL;
+  if (!s->finalized || !s->bound) return PSS_ESTATE;
+  if (s->cuda_bad) return PSS_ECUDA;
+  if (!fid_ok(s, field) || !s->fields[field].dynamic) return PSS_EINVAL;
+  const int slot = s->dyn_slot[field];
+  return (s->prec == PSS_F32) ? do_get_fourier<float>(s, slot, out, on_device)
+                              : do_get_fourier<double>(s, slot, out, on_device);
+}
+
+int pss_debug_noise(pss_system *s, int field, uint64_t step, uint32_t *bits, void *z) {
+  if (!s) return PSS_EINVAL;
+  if (!s->finalized || !s->bound) return PSS_ESTATE;
+  if (s->cuda_bad) return PSS_ECUDA;
+  if (!fid_ok(s, field)) return PSS_EINVAL;
+  return (s->prec == PSS_F32) ? do_debug_noise<float>(s, field, step, bits, z)
+                              : do_debug_noise<double>(s, field, step, bits, z);
+}
+
+int pss_profile_step(pss_system *s, int64_t nsteps, double ms_per_launch[3], int64_t launches[3]) {
+  if (!s || nsteps < 0 || nsteps > 4096 || !ms_per_launch || !launches) return PSS_EINVAL;
+  if (!s->finalized || !s->bound) return PSS_ESTATE;
+  if (s->cuda_bad) return PSS_ECUDA;
+  if (s->ndim == 1) return PSS_EUNSUPPORTED;
+  int rc = (s->prec == PSS_F32) ? do_steps<float>(s, 0) : do_steps<double>(s, 0);
+  /* make sure the prologue (if any) is not inside the profiled region */
+  if (s->P.nfac > 0 && !s->psix_valid) {
+    rc = (s->prec == PSS_F32) ? launch_update<float>(s, 1, s->step) : launch_update<double>(s, 1, s->step);
+    if (rc != PSS_OK) return rc;
+    s->psix_valid = true;
+  }
+  s->prof_on = true;
+  rc = (s->prec == PSS_F32) ? do_steps<float>(s, nsteps) : do_steps<double>(s, nsteps);
+  s->prof_on = false;
+  cudaError_t e = cudaStreamSynchronize(s->stream);
+  double sum[3] = {0, 0, 0};
+  int64_t cnt[3] = {0, 0, 0};
+  for (size_t i = 0; i < s->prof_kind.size() && 2 * i + 1 < s->prof_ev.size(); ++i) {
+    float ms = 0.f;
+    if (e == cudaSuccess && cudaEventElapsedTime(&ms, s->prof_ev[2 * i], s->prof_ev[2 * i + 1]) == cudaSuccess) {
+      sum[s->prof_kind[i]] += ms;
+      cnt[s->prof_kind[i]] += 1;
+    }
+  }
+  for (cudaEvent_t ev : s->prof_ev) cudaEventDestroy(ev);
+  s->prof_ev.clear();
+  s->prof_kind.clear();
+  for (int k = 0; k < 3; ++k) { ms_per_launch[k] = cnt[k] ? sum[k] / (double)cnt[k] : 0.0; launches[k] = cnt[k]; }
+  if (e != cudaSuccess) return cuda_fail(s, e, "pss_profile_step");
+  return rc;
+}
+
+uint64_t pss_launch_count(const pss_system *s) { return s ? s->launches : 0; }
+
+double pss_model_bytes_per_step(const pss_system *s, int pruned) {
+  if (!s || !s->finalized) return 0.0;
+  const Program &P = s->P;
+  const double S = (double)s->N * (double)s->rsize;
+  if (s->ndim == 1) return 2.0 * P.ndyn * S;
+  double c1 = 0.0, c2 = 0.0; /* sum over factors of the kept fraction per axis, and its square */
+  for (int f = 0; f < P.nfac; ++f) {
+    double c = 1.0;
+    if (pruned && P.dealias != PSS_DEALIAS_OFF)
+      c = 2.0 / (double)((P.dealias == PSS_DEALIAS_TWO_THIRDS ? 2 : P.fac[f].order) + 1);
+    c1 += c;
+    c2 += c * c;
+  }
+  if (s->ndim == 2) return S * (2.0 * P.ndyn + 2.0 * P.ngrp + 2.0 * c1);
+  return S * (2.0 * P.ndyn + 4.0 * P.ngrp + 2.0 * c2 + 2.0 * c1);
+}
+
+uint64_t pss_step_count(const pss_system *s) { return s ? s->step : 0; }
+
+const char *pss_strerror(int code) {
+  switch (code) {
+    case PSS_OK: return "ok";
+    case PSS_EINVAL: return "invalid argument";
+    case PSS_EUNSUPPORTED: return "unsupported configuration";
+    case PSS_ESTATE: return "call made in the wrong state";
+    case PSS_ECUDA: return "CUDA error (see pss_last_cuda_error)";
+    default: return "unknown error";
+  }
+}
+
+const char *pss_last_cuda_error(const pss_system *s) { return s ? s->cuda_msg.c_str() : ""; }
+
+void pss_destroy(pss_system *s) { delete s; }
+
+} /* extern "C" */

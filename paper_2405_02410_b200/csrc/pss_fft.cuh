@@ -1,0 +1,195 @@
+/*
+ * pss_fft.cuh — in-shared-memory FFT building blocks (sm_100a).
+ *
+ * A line of n = prod R_i complex points lives in shared memory, W lines interleaved:
+ * element (j, c) at buf[j*W + c].  Transforms are done IN PLACE without any reordering pass:
+ *   fft_dif : natural order in  -> digit-reversed order out   (decimation in frequency)
+ *   fft_dit : digit-reversed in -> natural order out           (its exact transpose)
+ * The callers pair them so the digit-reversed order only ever meets pointwise work, which does
+ * not care about order (transform, multiply pointwise, transform back).
+ * Radix-R butterflies (R in 2,4,8,16) run in registers; one __syncthreads between passes.
+ * Twiddles come from a table tw[j] = exp(-2 pi i j / n) computed on the host in long double.
+ */
+#ifndef PSS_FFT_CUH
+#define PSS_FFT_CUH
+#include <cuda_runtime.h>
+#include "pss_program.h"
+
+template <typename T> struct cplx_of;
+template <> struct cplx_of<float> { typedef float2 type; };
+template <> struct cplx_of<double> { typedef double2 type; };
+
+template <typename C, typename T> __device__ __forceinline__ C mk(T x, T y) { C r; r.x = x; r.y = y; return r; }
+template <typename C> __device__ __forceinline__ C cadd(C a, C b) { a.x += b.x; a.y += b.y; return a; }
+template <typename C> __device__ __forceinline__ C csub(C a, C b) { a.x -= b.x; a.y -= b.y; return a; }
+template <typename C> __device__ __forceinline__ C cmul(C a, C b) {
+  C r; r.x = a.x * b.x - a.y * b.y; r.y = a.x * b.y + a.y * b.x; return r;
+}
+/* a * conj(b) */
+template <typename C> __device__ __forceinline__ C cmulc(C a, C b) {
+  C r; r.x = a.x * b.x + a.y * b.y; r.y = a.y * b.x - a.x * b.y; return r;
+}
+
+/* multiply by exp(SGN * 2 pi i * J / LEN) for compile-time J, LEN (LEN <= 16) */
+template <int SGN, typename C> __device__ __forceinline__ C mul_root16(C d, int idx16) {
+  /* idx16 = J * 16 / LEN in [0, 8) */
+  typedef decltype(d.x) T;
+  const T c1 = (T)0.92387953251128675613, s1 = (T)0.38268343236508977173, h = (T)0.70710678118654752440;
+  T wr, wi;
+  switch (idx16) {
+    case 0: return d;
+    case 4: { C r; if (SGN < 0) { r.x = d.y; r.y = -d.x; } else { r.x = -d.y; r.y = d.x; } return r; }
+    case 1: wr = c1; wi = s1; break;
+    case 2: wr = h; wi = h; break;
+    case 3: wr = s1; wi = c1; break;
+    case 5: wr = -s1; wi = c1; break;
+    case 6: wr = -h; wi = h; break;
+    default: wr = -c1; wi = s1; break; /* 7 */
+  }
+  if (SGN < 0) wi = -wi;
+  C r; r.x = d.x * wr - d.y * wi; r.y = d.x * wi + d.y * wr; return r;
+}
+
+__host__ __device__ constexpr int bitrev_c(int i, int bits) {
+  int r = 0;
+  for (int b = 0; b < bits; ++b) r |= ((i >> b) & 1) << (bits - 1 - b);
+  return r;
+}
+
+/* R-point DFT in registers, natural in -> natural out, X[m] = sum_k v[k] exp(SGN 2 pi i m k / R) */
+template <int LGR, int SGN, typename C> __device__ __forceinline__ void dft_reg(C *v) {
+  constexpr int R = 1 << LGR;
+#pragma unroll
+  for (int len = R; len >= 2; len >>= 1) {
+    const int half = len >> 1;
+#pragma unroll
+    for (int blk = 0; blk < R; blk += len) {
+#pragma unroll
+      for (int j = 0; j < half; ++j) {
+        const C a = v[blk + j], b = v[blk + j + half];
+        v[blk + j] = cadd(a, b);
+        v[blk + j + half] = mul_root16<SGN>(csub(a, b), j * (16 / len));
+      }
+    }
+  }
+  C t[R];
+#pragma unroll
+  for (int i = 0; i < R; ++i) t[bitrev_c(i, LGR)] = v[i];
+#pragma unroll
+  for (int i = 0; i < R; ++i) v[i] = t[i];
+}
+
+/* digit reversal between smem slot p and frequency/time index f (see header) */
+__device__ __forceinline__ int geo_rev(const Geo &g, int p) { /* slot -> index */
+  int f = 0, sh = 0, lgrem = 0;
+#pragma unroll
+  for (int q = 0; q < 4; ++q) if (q < g.nr) lgrem += g.lg[q];
+#pragma unroll
+  for (int q = 0; q < 4; ++q) {
+    if (q < g.nr) {
+      lgrem -= g.lg[q];
+      const int m = (p >> lgrem) & ((1 << g.lg[q]) - 1);
+      f |= m << sh;
+      sh += g.lg[q];
+    }
+  }
+  return f;
+}
+__device__ __forceinline__ int geo_slot(const Geo &g, int f) { /* index -> slot */
+  int p = 0, lgrem = 0;
+#pragma unroll
+  for (int q = 0; q < 4; ++q) if (q < g.nr) lgrem += g.lg[q];
+#pragma unroll
+  for (int q = 0; q < 4; ++q) {
+    if (q < g.nr) {
+      lgrem -= g.lg[q];
+      const int m = f & ((1 << g.lg[q]) - 1);
+      f >>= g.lg[q];
+      p |= m << lgrem;
+    }
+  }
+  return p;
+}
+
+/* one radix-2^LGR pass over `ncol` interleaved columns: element (j, c) at buf[j*rs + c], c < ncol <= rs
+ * (several buffers of W columns each sit side by side in one row of rs columns).  lgL = log2 of the current sub-length L, lgn = log2 n.
+ * DIT = false: butterfly then twiddle (DIF).  DIT = true: twiddle then butterfly. */
+template <int LGR, int SGN, bool DIT, typename T>
+__device__ __forceinline__ void fft_pass(typename cplx_of<T>::type *buf, const typename cplx_of<T>::type *__restrict__ tw,
+                                         int lgn, int lgL, int ncol, int rs) {
+  typedef typename cplx_of<T>::type C;
+  constexpr int R = 1 << LGR;
+  const int lgLs = lgL - LGR;          /* log2 of the leg stride L/R */
+  const int nb = (1 << (lgn - LGR));   /* butterflies per column     */
+  const int total = nb * ncol;
+  for (int idx = threadIdx.x; idx < total; idx += blockDim.x) {
+    const int c = idx % ncol;
+    const int b = idx / ncol;
+    const int i = b & ((1 << lgLs) - 1);
+    const int blk = b >> lgLs;
+    C *p = buf + (size_t)((blk << lgL) + i) * rs + c;
+    const int ls = rs << lgLs;
+    const int tws = i << (lgn - lgL);  /* twiddle index step: w_L^i = tw[i * n/L] */
+    C v[R];
+#pragma unroll
+    for (int k = 0; k < R; ++k) v[k] = p[k * ls];
+    if (DIT) {
+#pragma unroll
+      for (int m = 1; m < R; ++m) {
+        const C w = __ldg(tw + m * tws);
+        v[m] = (SGN < 0) ? cmul(v[m], w) : cmulc(v[m], w);
+      }
+    }
+    dft_reg<LGR, SGN>(v);
+    if (!DIT) {
+#pragma unroll
+      for (int m = 1; m < R; ++m) {
+        const C w = __ldg(tw + m * tws);
+        v[m] = (SGN < 0) ? cmul(v[m], w) : cmulc(v[m], w);
+      }
+    }
+#pragma unroll
+    for (int k = 0; k < R; ++k) p[k * ls] = v[k];
+  }
+}
+
+template <int SGN, bool DIT, typename T>
+__device__ __forceinline__ void fft_pass_any(int lgr, typename cplx_of<T>::type *buf,
+                                             const typename cplx_of<T>::type *__restrict__ tw, int lgn, int lgL, int ncol, int rs) {
+  switch (lgr) {
+    case 1: fft_pass<1, SGN, DIT, T>(buf, tw, lgn, lgL, ncol, rs); break;
+    case 2: fft_pass<2, SGN, DIT, T>(buf, tw, lgn, lgL, ncol, rs); break;
+    case 3: fft_pass<3, SGN, DIT, T>(buf, tw, lgn, lgL, ncol, rs); break;
+    default: fft_pass<4, SGN, DIT, T>(buf, tw, lgn, lgL, ncol, rs); break;
+  }
+}
+
+/* natural -> digit-reversed.  Caller guarantees a __syncthreads() before; one is issued after. */
+template <int SGN, typename T>
+__device__ __forceinline__ void fft_dif(const Geo &g, typename cplx_of<T>::type *buf,
+                                        const typename cplx_of<T>::type *__restrict__ tw, int ncol, int rs) {
+  int lgn = 0;
+  for (int q = 0; q < g.nr; ++q) lgn += g.lg[q];
+  int lgL = lgn;
+  for (int q = 0; q < g.nr; ++q) {
+    fft_pass_any<SGN, false, T>(g.lg[q], buf, tw, lgn, lgL, ncol, rs);
+    lgL -= g.lg[q];
+    __syncthreads();
+  }
+}
+
+/* digit-reversed -> natural.  Caller guarantees a __syncthreads() before; one is issued after. */
+template <int SGN, typename T>
+__device__ __forceinline__ void fft_dit(const Geo &g, typename cplx_of<T>::type *buf,
+                                        const typename cplx_of<T>::type *__restrict__ tw, int ncol, int rs) {
+  int lgn = 0;
+  for (int q = 0; q < g.nr; ++q) lgn += g.lg[q];
+  int lgL = 0;
+  for (int q = g.nr - 1; q >= 0; --q) {
+    lgL += g.lg[q];
+    fft_pass_any<SGN, true, T>(g.lg[q], buf, tw, lgn, lgL, ncol, rs);
+    __syncthreads();
+  }
+}
+
+#endif

@@ -1,0 +1,491 @@
+/*
+ * pss_kernels.cuh — the kernels of the time step on the internal layout.
+ *
+ * INTERNAL LAYOUT (x slowest, last axis fastest):  arr[kx][y][z] (3D), arr[kx][y] (2D), with
+ * kx = 0..nx/2.  "rows" below are the r = y*nz + z positions that share one kx.  The state phi_q is
+ * kept in Fourier space; real space exists only inside k_rows' shared memory.
+ *
+ * One 2D step is two kernels:
+ *   k_rows   : for a tile of rows: C2R along x of every de-aliased factor (two real rows ride one
+ *              complex transform), the real-space products summed per group, R2C
+ *              along x.
+ *   k_update : for a tile of contiguous last-axis lines: forward FFT of the groups, outer operators
+ *              + explicit linear terms (Eq. 15), noise (Eq. 16), the implicit update (Eq. 18), then
+ *              for the NEXT step the factor operators, the de-aliasing mask
+ *               and the inverse FFT along the last axis.
+ * 3D adds k_mid (the y axis) between them in each direction.
+ */
+#ifndef PSS_KERNELS_CUH
+#define PSS_KERNELS_CUH
+#include "pss_pointwise.cuh"
+
+template <typename T> struct UpdArgs {
+  typename cplx_of<T>::type *state; /* [ndyn][M] */
+  typename cplx_of<T>::type *psix;  /* [nfac][M] */
+  typename cplx_of<T>::type *phat;  /* [ngrp][M] */
+  const typename cplx_of<T>::type *tw;
+  long long M;
+  int n;      /* last-axis length */
+  int nlines; /* nxh (2D) or nxh*ny (3D) */
+  int W;      /* lines per block */
+  int prologue;
+  unsigned long long step;
+  Geo geo;
+};
+
+/* ------------------------------------------------------------------------------------------ */
+template <typename T>
+__global__ void __launch_bounds__(256) k_update(const __grid_constant__ Program P, const UpdArgs<T> A) {
+  typedef typename cplx_of<T>::type C;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  C *sm = reinterpret_cast<C *>(smem_raw);
+  const int n = A.n, W = A.W;
+  const int line0 = blockIdx.x * W;
+  const int nl = min(W, A.nlines - line0);
+  const int nb0 = max(P.ngrp, P.ndyn);
+  const int RS = (nb0 + (P.nfac > 1 ? 1 : 0)) * W; /* columns per smem row */
+  const int tid = threadIdx.x, nt = blockDim.x;
+  const int ny3 = (P.ndim == 3) ? P.n[1] : 1;
+
+  /* ---- phase A: forward FFT of the groups along the last axis ---- */
+  if (!A.prologue) {
+    if (P.ngrp > 0) {
+      for (int g = 0; g < P.ngrp; ++g) {
+        const C *src = A.phat + (size_t)g * A.M + (size_t)line0 * n;
+        for (int idx = tid; idx < n * W; idx += nt) {
+          const int c = idx / n, j = idx - c * n;
+          sm[(size_t)j * RS + g * W + c] = (c < nl) ? src[(size_t)c * n + j] : mk<C, T>((T)0, (T)0);
+        }
+      }
+      __syncthreads();
+      fft_dif<-1, T>(A.geo, sm, A.tw, P.ngrp * W, RS);
+    }
+  }
+  /* ---- phase B: Eq. 15 + Eq. 16 + Eq. 18 per mode, natural order over k (coalesced state access) ---- */
+  for (int idx = tid; idx < n * W; idx += nt) {
+    const int c = idx / n, k = idx - c * n;
+    if (c >= nl) continue;
+    const int line = line0 + c;
+    const int slot = geo_slot(A.geo, k);
+    C *srow = sm + (size_t)slot * RS + c;
+    C phi[PSS_P_MAX_DYN];
+#pragma unroll
+    for (int i = 0; i < PSS_P_MAX_DYN; ++i)
+      phi[i] = (i < P.ndyn) ? A.state[(size_t)i * A.M + (size_t)line * n + k] : mk<C, T>((T)0, (T)0);
+    if (!A.prologue) {
+      int k0, k1, k2;
+      if (P.ndim == 3) { k0 = line / ny3; k1 = line - k0 * ny3; k2 = k; } else { k0 = line; k1 = k; k2 = 0; }
+      const ModeQ<T> mq = make_mode<T>(P, k0, k1, k2);
+      C out[PSS_P_MAX_DYN];
+#pragma unroll
+      for (int i = 0; i < PSS_P_MAX_DYN; ++i) {
+        if (i < P.ndyn) {
+          const DDyn &d = P.dyn[i];
+          C N = mk<C, T>((T)0, (T)0);
+          for (int g = 0; g < P.ngrp; ++g)
+            if (P.grp[g].target == i) N = cadd(N, cmul(eval_op<T>(P.grp[g].outer, mq), srow[g * W]));
+          for (int e = d.lin_beg; e < d.lin_end; ++e) N = cadd(N, cmul(eval_op<T>(P.lin[e], mq), sel4(phi, P.lin[e].src)));
+          C L = mk<C, T>((T)0, (T)0);
+          for (int e = d.lhs_beg; e < d.lhs_end; ++e) L = csub(L, eval_op<T>(P.lin[e], mq));
+          C num = mk<C, T>(phi[i].x + (T)P.dt * N.x, phi[i].y + (T)P.dt * N.y);
+          if (d.noisy) {
+            const T amp = noise_amp<T>(d, mq);
+            const C z = noise_z<T>(P, d.field_id, A.step, k0, k1, k2);
+            num.x += amp * z.x;
+            num.y += amp * z.y;
+          }
+          const C den = mk<C, T>((T)1 - (T)P.dt * L.x, -(T)P.dt * L.y);
+          const T id = (T)1 / (den.x * den.x + den.y * den.y);
+          const C q = cmulc(num, den);
+          out[i] = mk<C, T>(q.x * id, q.y * id);
+        } else {
+          out[i] = mk<C, T>((T)0, (T)0);
+        }
+      }
+#pragma unroll
+      for (int i = 0; i < PSS_P_MAX_DYN; ++i)
+        if (i < P.ndyn) {
+          A.state[(size_t)i * A.M + (size_t)line * n + k] = out[i];
+          srow[i * W] = out[i];
+        }
+    } else {
+#pragma unroll
+      for (int i = 0; i < PSS_P_MAX_DYN; ++i)
+        if (i < P.ndyn) srow[i * W] = phi[i];
+    }
+  }
+  __syncthreads();
+  /* ---- phase C: factor operators + mask + inverse FFT along the last axis, one factor at a time ---- */
+  for (int f = 0; f < P.nfac; ++f) {
+    const DFactor &F = P.fac[f];
+    const int wb = (f == P.nfac - 1) ? 0 : nb0; /* work buffer; the last factor may overwrite buffer 0 */
+    /* which of this block's lines survive the mask on their own (slow) axes? (block-uniform) */
+    unsigned keepmask = 0;
+    for (int c = 0; c < nl; ++c) {
+      const int line = line0 + c;
+      bool kp;
+      if (P.ndim == 3) {
+        const int k0 = line / ny3, k1 = line - k0 * ny3;
+        kp = keep_axis(P.dealias, F.order, k0, P.n[0]) && keep_axis(P.dealias, F.order, k1, P.n[1]);
+      } else {
+        kp = keep_axis(P.dealias, F.order, line, P.n[0]);
+      }
+      if (kp) keepmask |= 1u << c;
+    }
+    if (keepmask == 0) continue; /* the whole tile is masked: psix stays zero (zeroed at bind) */
+    for (int idx = tid; idx < n * W; idx += nt) {
+      const int c = idx % W, s = idx / W;
+      C *srow = sm + (size_t)s * RS + c;
+      C v = mk<C, T>((T)0, (T)0);
+      if ((keepmask >> c) & 1u) {
+        const int k = geo_rev(A.geo, s);
+        if (keep_axis(P.dealias, F.order, k, n)) {
+          const int line = line0 + c;
+          int k0, k1, k2;
+          if (P.ndim == 3) { k0 = line / ny3; k1 = line - k0 * ny3; k2 = k; } else { k0 = line; k1 = k; k2 = 0; }
+          const ModeQ<T> mq = make_mode<T>(P, k0, k1, k2);
+          C phi[PSS_P_MAX_DYN];
+#pragma unroll
+          for (int i = 0; i < PSS_P_MAX_DYN; ++i) phi[i] = (i < P.ndyn) ? srow[i * W] : mk<C, T>((T)0, (T)0);
+          for (int e = F.lin_beg; e < F.lin_end; ++e) v = cadd(v, cmul(eval_op<T>(P.lin[e], mq), sel4(phi, P.lin[e].src)));
+          v.x *= (T)P.invN;
+          v.y *= (T)P.invN;
+        }
+      }
+      srow[wb * W] = v;
+    }
+    __syncthreads();
+    fft_dit<+1, T>(A.geo, sm + wb * W, A.tw, W, RS);
+    C *dst = A.psix + (size_t)f * A.M + (size_t)line0 * n;
+    for (int idx = tid; idx < n * W; idx += nt) {
+      const int c = idx / n, j = idx - c * n;
+      if ((keepmask >> c) & 1u) dst[(size_t)c * n + j] = sm[(size_t)j * RS + wb * W + c];
+    }
+    __syncthreads();
+  }
+}
+
+/* ------------------------------------------------------------------------------------------ */
+template <typename T> struct RowArgs {
+  const typename cplx_of<T>::type *psix; /* [nfac][M]  (kx, r) */
+  typename cplx_of<T>::type *phat;       /* [ngrp][M]           */
+  const typename cplx_of<T>::type *tw;
+  long long M;
+  long long R; /* rows per kx: ny*nz */
+  int nx;
+  int Wc;      /* complex columns per block = row pairs */
+  Geo geo;
+};
+
+template <typename T>
+__global__ void __launch_bounds__(256) k_rows(const __grid_constant__ Program P, const RowArgs<T> A) {
+  typedef typename cplx_of<T>::type C;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  C *sm = reinterpret_cast<C *>(smem_raw);
+  const int nx = A.nx, nxh = nx / 2 + 1, Wc = A.Wc;
+  const int RS = (P.nfac + (P.ngrp > 1 ? 1 : 0)) * Wc;
+  const long long r0 = (long long)blockIdx.x * (2 * Wc);
+  const int tid = threadIdx.x, nt = blockDim.x;
+  const C zero = mk<C, T>((T)0, (T)0);
+
+  /* zero, then Hermitian-extend the kept part of every factor: Z_k = A_k + i B_k (rows r, r+1) */
+  for (int idx = tid; idx < nx * RS; idx += nt) sm[idx] = zero;
+  __syncthreads();
+  for (int f = 0; f < P.nfac; ++f) {
+    int cut = nxh; /* number of kept kx */
+    if (P.dealias != 2) {
+      const int nn = (P.dealias == 1 ? 2 : P.fac[f].order) + 1;
+      cut = (nx + nn - 1) / nn; /* kx kept iff nn*kx < nx */
+      if (cut > nxh) cut = nxh;
+    }
+    const C *src = A.psix + (size_t)f * A.M + r0;
+    for (int idx = tid; idx < cut * Wc; idx += nt) {
+      const int c = idx % Wc, kx = idx / Wc;
+      const C *p = src + (size_t)kx * A.R + 2 * c;
+      C a = p[0], b = p[1];
+      if (kx == 0 || 2 * kx == nx) { a.y = (T)0; b.y = (T)0; } /* C2R keeps the real part there */
+      sm[(size_t)kx * RS + f * Wc + c] = mk<C, T>(a.x - b.y, a.y + b.x);
+      if (kx > 0 && 2 * kx < nx) sm[(size_t)(nx - kx) * RS + f * Wc + c] = mk<C, T>(a.x + b.y, b.x - a.y);
+    }
+  }
+  __syncthreads();
+  if (P.nfac > 0) fft_dif<+1, T>(A.geo, sm, A.tw, P.nfac * Wc, RS);
+  /* real-space products per group, forward transform, Hermitian split */
+  for (int g = 0; g < P.ngrp; ++g) {
+    const DGroup &G = P.grp[g];
+    const int wb = (g == P.ngrp - 1) ? 0 : P.nfac;
+    for (int idx = tid; idx < nx * Wc; idx += nt) {
+      const int c = idx % Wc, s = idx / Wc;
+      const C *srow = sm + (size_t)s * RS + c;
+      T pa = (T)0, pb = (T)0;
+      for (int t = G.term_beg; t < G.term_end; ++t) {
+        const DTerm &tm = P.term[t];
+        T ta = (T)tm.coef, tb = (T)tm.coef;
+        for (int i = 0; i < tm.nf; ++i) {
+          const C v = srow[tm.f[i] * Wc];
+          ta *= v.x;
+          tb *= v.y;
+        }
+        pa += ta;
+        pb += tb;
+      }
+      sm[(size_t)s * RS + wb * Wc + c] = mk<C, T>(pa, pb);
+    }
+    __syncthreads();
+    fft_dit<-1, T>(A.geo, sm + wb * Wc, A.tw, Wc, RS);
+    C *dst = A.phat + (size_t)g * A.M + r0;
+    for (int idx = tid; idx < nxh * Wc; idx += nt) {
+      const int c = idx % Wc, kx = idx / Wc;
+      const C z = sm[(size_t)kx * RS + wb * Wc + c];
+      const C zm = sm[(size_t)((nx - kx) & (nx - 1)) * RS + wb * Wc + c];
+      const T h = (T)0.5;
+      C *p = dst + (size_t)kx * A.R + 2 * c;
+      p[0] = mk<C, T>(h * (z.x + zm.x), h * (z.y - zm.y));
+      p[1] = mk<C, T>(h * (z.y + zm.y), h * (zm.x - z.x));
+    }
+    __syncthreads();
+  }
+}
+
+/* ------------------------------------------------------------------------------------------ */
+/* middle (y) axis of 3D arrays arr[b][kx][y][z]: tile = (kx, W contiguous z), in place, natural order */
+template <typename T> struct MidArgs {
+  typename cplx_of<T>::type *arr;
+  const typename cplx_of<T>::type *tw;
+  long long M;
+  int ny, nz, W;
+  int kx_count; /* lines with kx >= kx_count are skipped (de-aliased away) */
+  int nx;
+  int nn[PSS_P_MAX_FAC]; /* per batch entry: order+1 of the de-aliasing rule, 0 = no mask.  Rows ky and lines
+                            kx outside the kept band were never written by k_update: read them as zero */
+  Geo geo;
+};
+
+template <int SGN, typename T> __global__ void __launch_bounds__(256) k_mid(const MidArgs<T> A) {
+  typedef typename cplx_of<T>::type C;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  C *sm = reinterpret_cast<C *>(smem_raw);
+  const int W = A.W, ny = A.ny;
+  const int kx = blockIdx.y;
+  if (kx >= A.kx_count) return;
+  const int nn = A.nn[blockIdx.z];
+  if (nn && nn * kx >= A.nx) return;
+  C *base = A.arr + (size_t)blockIdx.z * A.M + (size_t)kx * ny * A.nz + (size_t)blockIdx.x * W;
+  for (int idx = threadIdx.x; idx < ny * W; idx += blockDim.x) {
+    const int c = idx % W, j = idx / W;
+    int a = signed_index(j, ny);
+    a = a < 0 ? -a : a;
+    sm[idx] = (nn && nn * a >= ny) ? mk<C, T>((T)0, (T)0) : base[(size_t)j * A.nz + c];
+  }
+  __syncthreads();
+  fft_dif<SGN, T>(A.geo, sm, A.tw, W, W);
+  for (int idx = threadIdx.x; idx < ny * W; idx += blockDim.x) {
+    const int c = idx % W, s = idx / W;
+    base[(size_t)geo_rev(A.geo, s) * A.nz + c] = sm[idx];
+  }
+}
+
+/* last axis, contiguous lines, in place, natural order (set/get paths only) */
+template <typename T> struct LastArgs {
+  typename cplx_of<T>::type *arr;
+  const typename cplx_of<T>::type *tw;
+  int n, nlines;
+  Geo geo;
+};
+
+template <int SGN, typename T> __global__ void __launch_bounds__(256) k_last(const LastArgs<T> A) {
+  typedef typename cplx_of<T>::type C;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  C *sm = reinterpret_cast<C *>(smem_raw);
+  const int n = A.n;
+  C *base = A.arr + (size_t)blockIdx.x * n;
+  for (int j = threadIdx.x; j < n; j += blockDim.x) sm[j] = base[j];
+  __syncthreads();
+  fft_dif<SGN, T>(A.geo, sm, A.tw, 1, 1);
+  for (int j = threadIdx.x; j < n; j += blockDim.x) base[j] = sm[geo_slot(A.geo, j)];
+}
+
+/* ------------------------------------------------------------------------------------------ */
+/* x axis between the USER layout (real, x fastest, then y, then z) and the internal layout.
+ * One block per pair of user rows (ndim >= 2) or per single row (1D).  DIR = -1: R2C, +1: C2R. */
+template <typename T> struct UserArgs {
+  T *real;                                /* user array               */
+  typename cplx_of<T>::type *arr;         /* internal [kx][y][z]      */
+  const typename cplx_of<T>::type *tw;
+  int nx, ny, nz, single;
+  double scale;
+  Geo geo;
+};
+
+template <int DIR, typename T> __global__ void __launch_bounds__(256) k_user_x(const UserArgs<T> A) {
+  typedef typename cplx_of<T>::type C;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  C *sm = reinterpret_cast<C *>(smem_raw);
+  const int nx = A.nx, nxh = nx / 2 + 1;
+  const long long R = (long long)A.ny * A.nz;
+  const long long ra = A.single ? blockIdx.x : 2ll * blockIdx.x, rb = ra + 1; /* user row ids z*ny + y */
+  const long long ia = (ra % A.ny) * A.nz + ra / A.ny;                          /* internal y*nz + z    */
+  const long long ib = A.single ? ia : (rb % A.ny) * A.nz + rb / A.ny;
+  if (DIR < 0) {
+    for (int x = threadIdx.x; x < nx; x += blockDim.x)
+      sm[x] = mk<C, T>(A.real[ra * nx + x], A.single ? (T)0 : A.real[rb * nx + x]);
+    __syncthreads();
+    fft_dif<-1, T>(A.geo, sm, A.tw, 1, 1);
+    for (int kx = threadIdx.x; kx < nxh; kx += blockDim.x) {
+      const C z = sm[geo_slot(A.geo, kx)];
+      const C zm = sm[geo_slot(A.geo, (nx - kx) & (nx - 1))];
+      const T h = (T)0.5;
+      A.arr[(size_t)kx * R + ia] = mk<C, T>(h * (z.x + zm.x), h * (z.y - zm.y));
+      if (!A.single) A.arr[(size_t)kx * R + ib] = mk<C, T>(h * (z.y + zm.y), h * (zm.x - z.x));
+    }
+  } else {
+    for (int kx = threadIdx.x; kx < nxh; kx += blockDim.x) {
+      C a = A.arr[(size_t)kx * R + ia];
+      C b = A.single ? mk<C, T>((T)0, (T)0) : A.arr[(size_t)kx * R + ib];
+      if (kx == 0 || 2 * kx == nx) { a.y = (T)0; b.y = (T)0; }
+      sm[kx] = mk<C, T>(a.x - b.y, a.y + b.x);
+      if (kx > 0 && 2 * kx < nx) sm[nx - kx] = mk<C, T>(a.x + b.y, b.x - a.y);
+    }
+    __syncthreads();
+    fft_dif<+1, T>(A.geo, sm, A.tw, 1, 1);
+    const T sc = (T)A.scale;
+    for (int x = threadIdx.x; x < nx; x += blockDim.x) {
+      const C z = sm[geo_slot(A.geo, x)];
+      A.real[ra * nx + x] = z.x * sc;
+      if (!A.single) A.real[rb * nx + x] = z.y * sc;
+    }
+  }
+}
+
+/* internal [kx][r] -> logical [r'][kx] (r' = z*ny + y) for pss_get_field_fourier */
+template <typename T>
+__global__ void k_to_logical(const typename cplx_of<T>::type *arr, typename cplx_of<T>::type *out, int nxh, int ny, int nz) {
+  const long long total = (long long)nxh * ny * nz;
+  for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < total; i += (long long)gridDim.x * blockDim.x) {
+    const int kx = (int)(i % nxh);
+    const long long rp = i / nxh;
+    const long long y = rp % ny, z = rp / ny;
+    out[i] = arr[(size_t)kx * ny * nz + y * nz + z];
+  }
+}
+
+/* noise test hook: Philox words and z per logical mode */
+template <typename T>
+__global__ void k_debug_noise(const __grid_constant__ Program P, int field, unsigned long long step, uint32_t *bits,
+                              typename cplx_of<T>::type *z) {
+  const long long total = (long long)P.nxh * P.n[1] * P.n[2];
+  for (long long m = blockIdx.x * (long long)blockDim.x + threadIdx.x; m < total; m += (long long)gridDim.x * blockDim.x) {
+    const int k0 = (int)(m % P.nxh);
+    const long long rp = m / P.nxh;
+    const int k1 = (int)(rp % P.n[1]), k2 = (int)(rp / P.n[1]);
+    if (bits) {
+      uint32_t w[4];
+      noise_block(P, field, step, m, w);
+      bits[4 * m] = w[0]; bits[4 * m + 1] = w[1]; bits[4 * m + 2] = w[2]; bits[4 * m + 3] = w[3];
+    }
+    if (z) z[m] = noise_z<T>(P, field, step, k0, k1, k2);
+  }
+}
+
+/* ------------------------------------------------------------------------------------------ */
+/* 1D: the whole lattice fits one CTA; nsteps full steps per launch, state in
+ * global memory (nxh complex per dynamic field), everything else in shared memory. */
+template <typename T> struct Step1dArgs {
+  typename cplx_of<T>::type *state; /* [ndyn][nxh] */
+  const typename cplx_of<T>::type *tw;
+  long long M;
+  int nx;
+  long long nsteps;
+  unsigned long long step0;
+  Geo geo;
+};
+
+template <typename T>
+__global__ void __launch_bounds__(256) k_step1d(const __grid_constant__ Program P, const Step1dArgs<T> A) {
+  typedef typename cplx_of<T>::type C;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  C *sm = reinterpret_cast<C *>(smem_raw);
+  const int nx = A.nx, nxh = nx / 2 + 1;
+  const int RS = P.nfac + P.ngrp;
+  const int tid = threadIdx.x, nt = blockDim.x;
+  const C zero = mk<C, T>((T)0, (T)0);
+  for (long long st = 0; st < A.nsteps; ++st) {
+    /* steps 1-3: factor operators, mask, C2R (imaginary row unused) */
+    for (int idx = tid; idx < nx * RS; idx += nt) sm[idx] = zero;
+    __syncthreads();
+    for (int kx = tid; kx < nxh; kx += nt) {
+      const ModeQ<T> mq = make_mode<T>(P, kx, 0, 0);
+      C phi[PSS_P_MAX_DYN];
+#pragma unroll
+      for (int i = 0; i < PSS_P_MAX_DYN; ++i) phi[i] = (i < P.ndyn) ? A.state[(size_t)i * A.M + kx] : zero;
+      for (int f = 0; f < P.nfac; ++f) {
+        const DFactor &F = P.fac[f];
+        if (!keep_axis(P.dealias, F.order, kx, nx)) continue;
+        C v = zero;
+        for (int e = F.lin_beg; e < F.lin_end; ++e) v = cadd(v, cmul(eval_op<T>(P.lin[e], mq), sel4(phi, P.lin[e].src)));
+        v.x *= (T)P.invN;
+        v.y *= (T)P.invN;
+        if (kx == 0 || 2 * kx == nx) v.y = (T)0;
+        sm[(size_t)kx * RS + f] = v;
+        if (kx > 0 && 2 * kx < nx) sm[(size_t)(nx - kx) * RS + f] = mk<C, T>(v.x, -v.y);
+      }
+    }
+    __syncthreads();
+    if (P.nfac > 0) fft_dif<+1, T>(A.geo, sm, A.tw, P.nfac, RS);
+    /* steps 3-4: products and R2C */
+    for (int idx = tid; idx < nx; idx += nt) {
+      C *srow = sm + (size_t)idx * RS;
+      for (int g = 0; g < P.ngrp; ++g) {
+        const DGroup &G = P.grp[g];
+        T pa = (T)0;
+        for (int t = G.term_beg; t < G.term_end; ++t) {
+          const DTerm &tm = P.term[t];
+          T ta = (T)tm.coef;
+          for (int i = 0; i < tm.nf; ++i) ta *= srow[tm.f[i]].x;
+          pa += ta;
+        }
+        srow[P.nfac + g] = mk<C, T>(pa, (T)0);
+      }
+    }
+    __syncthreads();
+    if (P.ngrp > 0) fft_dit<-1, T>(A.geo, sm + P.nfac, A.tw, P.ngrp, RS);
+    /* steps 5-6: noise and Eq. 18 */
+    for (int kx = tid; kx < nxh; kx += nt) {
+      const ModeQ<T> mq = make_mode<T>(P, kx, 0, 0);
+      const C *srow = sm + (size_t)kx * RS + P.nfac;
+      C phi[PSS_P_MAX_DYN], out[PSS_P_MAX_DYN];
+#pragma unroll
+      for (int i = 0; i < PSS_P_MAX_DYN; ++i) phi[i] = (i < P.ndyn) ? A.state[(size_t)i * A.M + kx] : zero;
+#pragma unroll
+      for (int i = 0; i < PSS_P_MAX_DYN; ++i) {
+        out[i] = zero;
+        if (i < P.ndyn) {
+          const DDyn &d = P.dyn[i];
+          C N = zero;
+          for (int g = 0; g < P.ngrp; ++g)
+            if (P.grp[g].target == i) N = cadd(N, cmul(eval_op<T>(P.grp[g].outer, mq), srow[g]));
+          for (int e = d.lin_beg; e < d.lin_end; ++e) N = cadd(N, cmul(eval_op<T>(P.lin[e], mq), sel4(phi, P.lin[e].src)));
+          C L = zero;
+          for (int e = d.lhs_beg; e < d.lhs_end; ++e) L = csub(L, eval_op<T>(P.lin[e], mq));
+          C num = mk<C, T>(phi[i].x + (T)P.dt * N.x, phi[i].y + (T)P.dt * N.y);
+          if (d.noisy) {
+            const T amp = noise_amp<T>(d, mq);
+            const C z = noise_z<T>(P, d.field_id, A.step0 + (unsigned long long)st, kx, 0, 0);
+            num.x += amp * z.x;
+            num.y += amp * z.y;
+          }
+          const C den = mk<C, T>((T)1 - (T)P.dt * L.x, -(T)P.dt * L.y);
+          const T id = (T)1 / (den.x * den.x + den.y * den.y);
+          const C q = cmulc(num, den);
+          out[i] = mk<C, T>(q.x * id, q.y * id);
+        }
+      }
+#pragma unroll
+      for (int i = 0; i < PSS_P_MAX_DYN; ++i)
+        if (i < P.ndyn) A.state[(size_t)i * A.M + kx] = out[i];
+    }
+    __syncthreads();
+  }
+}
+
+#endif

@@ -1,0 +1,91 @@
+/*
+ * pss_program.h — the frozen term list of one field system, as plain data handed to the kernels
+ * by value (a __grid_constant__ kernel parameter, < 4 KB).
+ *
+ * It restates PAPER.md:82-90 (Eq. 10-11): dynamic fields phi_i with an implicit operator L_i,
+ * intermediate fields psi_k that are operators applied to fields, and rhs terms
+ * M_ij prod_k psi_k^{n_k}.  Intermediate fields that are linear in the dynamic fields (all of
+ * BASELINE's workloads) are flattened on the host into sums of operator monomials acting directly on
+ * dynamic fields, so that the kernels evaluate them pointwise per mode from registers.
+ */
+#ifndef PSS_PROGRAM_H
+#define PSS_PROGRAM_H
+#include <stdint.h>
+
+#define PSS_P_MAX_DYN 4
+#define PSS_P_MAX_FAC 12
+#define PSS_P_MAX_GRP 8
+#define PSS_P_MAX_TERM 32
+#define PSS_P_MAX_LIN 96
+
+/* coef (q^2)^m |q|^-p prod_j (i q_j)^a[j] acting on dynamic field `src`.
+ * zflags bit j (j<3): the monomial is 0 at the Nyquist index of axis j (reading A9, applied link by
+ * link before flattening); bit 3: it is 0 at q = 0 (reading A10). */
+struct DOp {
+  double coef;
+  int8_t m, p;
+  int8_t a[3];
+  uint8_t zflags;
+  int8_t src;
+  int8_t pad_;
+};
+
+/* one product term of a group: coef * prod_{i<nf} factor[f[i]](x) */
+struct DTerm {
+  double coef;
+  int8_t nf;
+  int8_t f[4];
+  int8_t pad_[3];
+};
+
+/* a field that enters products of order >= 2: its de-aliased copy is transformed */
+struct DFactor {
+  int16_t lin_beg, lin_end; /* psi_q = sum_{e in [beg,end)} lin[e](q) * phi_{src_e}(q) */
+  int16_t order;            /* highest order n of a product it appears in           */
+  int16_t pad_;
+};
+
+/* all product terms with the same target field and the same outer operator are summed in real
+ * space before the forward transform (the transform is linear) */
+struct DGroup {
+  DOp outer; /* coef = 1, src = target dynamic slot */
+  int16_t term_beg, term_end;
+  int16_t target;
+  int16_t pad_;
+};
+
+struct DDyn {
+  int16_t lhs_beg, lhs_end; /* L_q = - sum lin[e](q)                  (dt phi + lhs = rhs, A3) */
+  int16_t lin_beg, lin_end; /* explicit linear terms sum lin[e](q) phi_src(q)   (A8)          */
+  double noise_c;           /* 2 D dt N / dV                           (A1)                   */
+  int16_t noise_qpow;       /* a in D~ = D |q|^a                       (A13)                  */
+  int16_t noisy;
+  int32_t field_id;         /* user field id: enters the Philox counter                       */
+};
+
+struct Program {
+  int32_t ndim;
+  int32_t n[3];
+  int32_t nxh;
+  int32_t dealias;
+  double qs[3]; /* 2 pi / (n_j dx_j) */
+  double dt;
+  double invN;
+  uint32_t seed_lo, seed_hi;
+  int32_t ndyn, nfac, ngrp, nterm, nlin;
+  int32_t pad_;
+  DDyn dyn[PSS_P_MAX_DYN];
+  DFactor fac[PSS_P_MAX_FAC];
+  DGroup grp[PSS_P_MAX_GRP];
+  DTerm term[PSS_P_MAX_TERM];
+  DOp lin[PSS_P_MAX_LIN];
+};
+
+/* radix schedule of one in-shared-memory FFT of length n = prod R[i] */
+struct Geo {
+  int32_t n;
+  int32_t nr;
+  int32_t lg[4]; /* log2 of the radices, first DIF pass first */
+};
+
+#endif
