@@ -1,0 +1,336 @@
+#!/usr/bin/env python
+"""bench.py — timesteps/s and site-updates/s of the pseudo-spectral SPDE step on B200.
+
+    python bench.py --gpus N --steps K --warmup W [--workload modelb_1024] [--inner 500]
+    python bench.py --impl reference ...            # the CPU oracle, timed on the host cores
+
+One bench "step" is one call pss_step(inner): `inner` consecutive time steps of the whole hot path
+(k_rows + k_update per time step) on the workload's lattice.  The state of a time stepper is consumed by
+the next time step, so inside one bench step the working set is as warm as the workload makes it; BETWEEN
+timed bench steps L2 is flushed (a 256 MiB buffer is written), so every timed step starts cold.
+
+value      = timesteps/s with the state resident in HBM (sum over ranks; N > 1 runs independent replicas,
+             different seeds, no collective: "replicas only", DESIGN.md section Multi-GPU)
+e2e        = the same through the public API with HOST buffers: pss_set_field(host) -> pss_step(inner) ->
+             pss_get_field(host) inside the timed region
+roofline   = dominant kernel (by device time, from pss_profile_step's per-launch CUDA events): algorithmic
+             bytes per launch / mean launch duration against MEASURED_PEAKS.json's HBM copy bandwidth
+cpu_baseline = the oracle as it stands on the host cores, bounded sample
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+from paper_2405_02410_b200 import workloads as wl  # noqa: E402
+
+FALLBACK_HBM_GBS = 6650.0  # /opt/skills/guides/B200_PROFILING.md "FALLBACK"
+
+
+def measured_peak():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(p) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled during the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.lines = []
+        self.proc = None
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.lines:
+            parts = [p.strip() for p in ln.split(",")]
+            if len(parts) < 6:
+                continue
+            try:
+                sm.append(float(parts[0]))
+                mx.append(float(parts[1]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, parts[2:6]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def oracle_rate(cfg, prec, budget_s, max_steps):
+    """timesteps/s of the CPU oracle on a bounded sample: 1 warm-up step, then steps until budget_s."""
+    from oracle import opss
+    o, _ = wl.build(opss, cfg, prec=prec)
+    o.step(1)
+    n, t0 = 0, time.perf_counter()
+    while True:
+        o.step(1)
+        n += 1
+        el = time.perf_counter() - t0
+        if el >= budget_s or n >= max_steps:
+            break
+    cores = int(os.environ.get("OMP_NUM_THREADS", "0")) or (os.cpu_count() or 1)
+    return n / el, n, el, cores
+
+
+def run_reference(args, cfg, rank, world):
+    if rank != 0:
+        return
+    per = []
+    for _ in range(args.warmup):
+        pass  # the oracle has no warm state beyond its own first step (done inside oracle_rate)
+    sites = int(np.prod(cfg["n"]))
+    total_steps, total_t = 0, 0.0
+    cores = 1
+    for _ in range(args.steps):
+        r, n, el, cores = oracle_rate(cfg, args.prec, args.ref_budget / max(1, args.steps), 64)
+        per.append(r)
+        total_steps += n
+        total_t += el
+    v = total_steps / total_t
+    line = {
+        "impl": "reference", "metric": "timesteps/s", "value": v, "unit": "timesteps/s", "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * total_t / max(1, args.steps),
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "site_updates_per_s": v * sites,
+        "config": {"workload": args.workload, "lattice": list(cfg["n"]), "precision": args.prec,
+                   "note": "CPU oracle (oracle/opss.cpp) as it stands; each step is a bounded sample of oracle time steps"},
+        "cpu_baseline": {"value": v, "unit": "timesteps/s", "cores": cores, "kind": "oracle",
+                         "sample": "%d oracle time steps of %s in %.1f s" % (total_steps, args.workload, total_t)},
+        "e2e": {"value": v, "unit": "timesteps/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--inner", type=int, default=500, help="time steps per bench step (one pss_step call)")
+    ap.add_argument("--workload", default="modelb_1024")
+    ap.add_argument("--prec", default="f32")
+    ap.add_argument("--impl", default="pss", choices=["pss", "reference"])
+    ap.add_argument("--ref-budget", type=float, default=20.0, help="seconds of oracle work for the reference arm")
+    ap.add_argument("--cpu-budget", type=float, default=12.0, help="seconds of oracle work for cpu_baseline")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    cfg = wl.make_config(args.workload)
+
+    if args.impl == "reference":
+        run_reference(args, cfg, rank, world)
+        return
+
+    import torch
+    import torch.distributed as dist
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the product has no CPU fallback)")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    import paper_2405_02410_b200 as pss
+
+    # replicas only: every rank advances its own realisation (seed + rank), no data-path collective
+    cfg_r = dict(cfg)
+    cfg_r["seed"] = cfg["seed"] + rank
+    g, ids = wl.build(pss, cfg_r, prec=args.prec, device="cuda:%d" % local_rank)
+    dyn_names = list(cfg["ic"].keys())
+    sites = int(np.prod(cfg["n"]))
+    rsize = 4 if args.prec == "f32" else 8
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    stream = torch.cuda.current_stream(dev)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    def reset_state():
+        for name, arr in wl.initial_conditions(cfg_r, g.rdtype).items():
+            g.set_field(ids[name], arr)
+
+    # nematic (A20): the literal parameters blow up after ~400 steps -> re-seed before every bench step
+    reseed = cfg["model"] == "nematic"
+    inner = min(args.inner, 250) if reseed else args.inner
+
+    for _ in range(max(args.warmup, 0)):
+        if reseed:
+            reset_state()
+        g.step(inner)
+    barrier()
+
+    launches0 = g.launch_count
+    sampler = ClockSampler(local_rank) if rank == 0 else None
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    barrier()
+    launches_timed = 0
+    for i in range(args.steps):
+        if reseed:
+            reset_state()
+        flush.fill_(i & 0xff)  # L2 flush between timed steps (not timed)
+        l0 = g.launch_count
+        ev[i][0].record(stream)
+        g.step(inner)
+        ev[i][1].record(stream)
+        launches_timed += g.launch_count - l0
+    barrier()
+    ms = [a.elapsed_time(b) for a, b in ev]
+    total_ms = float(sum(ms))
+    clocks = sampler.stop() if sampler else None
+
+    # ---- e2e: host buffers through the public API, copies inside the timed region ----
+    host_in = {name: torch.from_numpy(arr).pin_memory() for name, arr in wl.initial_conditions(cfg_r, g.rdtype).items()}
+    host_out = {name: torch.empty_like(t).pin_memory() for name, t in host_in.items()}
+    e2e_steps = max(2, min(args.steps, 5))
+
+    def e2e_once():
+        for name in dyn_names:
+            g.set_field(ids[name], host_in[name].numpy())
+        g.step(inner)
+        for name in dyn_names:
+            g.get_field(ids[name], out=host_out[name].numpy())
+
+    e2e_once()
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        e2e_once()
+    torch.cuda.synchronize(dev)
+    e2e_s = time.perf_counter() - t0
+    finite = all(bool(np.isfinite(host_out[n].numpy()).all()) for n in dyn_names)
+
+    # ---- per-kernel device times (CUDA events around every launch) for the roofline of the dominant kernel ----
+    if reseed:
+        reset_state()
+    prof = g.profile_step(min(200, inner))
+    barrier()
+
+    # max over ranks of the timed totals; sum of units
+    t_total = torch.tensor([total_ms, e2e_s], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t_total, op=dist.ReduceOp.MAX)
+    total_ms, e2e_s = float(t_total[0]), float(t_total[1])
+    steps_all = world * args.steps * inner
+    value = steps_all / (total_ms * 1e-3)
+    e2e_value = world * e2e_steps * inner / e2e_s
+
+    if rank == 0:
+        peak, peak_src = measured_peak()
+        S = sites * rsize
+        b_alg = g.model_bytes_per_step(True)
+        b_model = g.model_bytes_per_step(False)
+        step_ms = total_ms / (args.steps * inner)
+        # dominant kernel by share of device time
+        shares = {k: v[0] * v[1] for k, v in prof.items() if v[1] > 0}
+        dom = max(shares, key=shares.get)
+        dom_ms = prof[dom][0]
+        P = g  # algorithmic bytes per launch of each kernel family
+        kb = kernel_bytes(cfg, S, g)
+        ach = kb[dom] / (dom_ms * 1e-3) / 1e9
+        line = {
+            "metric": "timesteps/s", "value": value, "unit": "timesteps/s", "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": args.prec, "data": "synthetic",
+            "site_updates_per_s": value * sites, "us_per_timestep": step_ms * 1e3,
+            "config": {"workload": args.workload, "lattice": list(cfg["n"]), "precision": args.prec,
+                       "timesteps_per_bench_step": inner, "parallelism": "replicas only (one realisation per GPU)",
+                       "l2": "flushed between timed bench steps (256 MiB written); inside a bench step the "
+                             "time stepper reuses its own state, as the workload does",
+                       "final_state_finite": finite},
+            "gpu_launches": int(launches_timed),
+            "clocks": clocks,
+            "e2e": {"value": e2e_value, "unit": "timesteps/s",
+                    "h2d_bytes_per_step": len(dyn_names) * S, "d2h_bytes_per_step": len(dyn_names) * S,
+                    "note": "pss_set_field(host) + pss_step(%d) + pss_get_field(host) per bench step" % inner},
+            "roofline": {"bound": "hbm", "kernel": dom, "achieved": ach, "peak": peak, "unit": "GB/s",
+                         "frac": ach / peak, "traffic": ncu_traffic(dom), "peak_source": peak_src,
+                         "algorithmic_bytes_per_launch": kb[dom], "launch_ms": dom_ms,
+                         "kernel_ms": {k: v[0] for k, v in prof.items() if v[1] > 0},
+                         "kernel_share": {k: shares[k] / sum(shares.values()) for k in shares}},
+            "roofline_step": {"B_alg_bytes": b_alg, "B_model_bytes": b_model,
+                              "achieved_alg_GBs": b_alg / (step_ms * 1e-3) / 1e9,
+                              "frac_alg": b_alg / (step_ms * 1e-3) / 1e9 / peak,
+                              "frac_model": b_model / (step_ms * 1e-3) / 1e9 / peak,
+                              "frac_alg_of_8TBs": b_alg / (step_ms * 1e-3) / 1e9 / 8000.0},
+        }
+        if not args.no_cpu_baseline and world == 1:
+            r, n, el, cores = oracle_rate(cfg, args.prec, args.cpu_budget, 64)
+            line["cpu_baseline"] = {"value": r, "unit": "timesteps/s", "cores": cores, "kind": "oracle",
+                                    "sample": "%d oracle time steps of %s after 1 warm-up step, %.1f s" % (n, args.workload, el)}
+        print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def kernel_bytes(cfg, S, g):
+    """algorithmic bytes per launch of each kernel family (pruned count, SURVEY.md 8(d) / DESIGN.md)."""
+    total = g.model_bytes_per_step(True)
+    ndim = len(cfg["n"])
+    model = cfg["model"]
+    # factor kept-fractions and counts follow from the term list; derive the split from the totals:
+    # rows   : sum_f c_f (read) + ngrp (write)
+    # update : ngrp (read) + 2 ndyn + sum_f c_f^(ndim-1) (write)
+    table = {"model_b": (1, 1, [0.5]), "kpz": (1, 1, [2 / 3.0] * ndim),
+             "nematic": (2, 2, [0.5, 0.5] + [2 / 3.0] * 7), "diffusion": (1, 0, [])}
+    ndyn, ngrp, cs = table[model]
+    rows = S * (sum(cs) + ngrp)
+    upd = S * (ngrp + 2 * ndyn + sum(c ** (ndim - 1) for c in cs))
+    mid = 0.0
+    if ndim == 3:
+        mid = (total - rows - upd) / 2.0  # two k_mid launches per step (forward on groups, inverse on factors)
+    return {"k_rows": rows, "k_update": upd, "k_mid": mid}
+
+
+def ncu_traffic(kernel):
+    """dram bytes per launch of the kernel from the committed ncu capture (profiles/), or None."""
+    p = os.path.join(ROOT, "profiles", "ncu_traffic.json")
+    try:
+        with open(p) as f:
+            return json.load(f).get(kernel)
+    except Exception:
+        return None
+
+
+if __name__ == "__main__":
+    main()
