@@ -243,7 +243,8 @@ def main():
     # ---- per-kernel device times (CUDA events around every launch) for the roofline of the dominant kernel ----
     if reseed:
         reset_state()
-    prof = g.profile_step(min(200, inner))
+    prof_n = min(200, inner)
+    prof = g.profile_step(prof_n)
     barrier()
 
     # max over ranks of the timed totals; sum of units
@@ -266,7 +267,7 @@ def main():
         dom = max(shares, key=shares.get)
         dom_ms = prof[dom][0]
         P = g  # algorithmic bytes per launch of each kernel family
-        kb = kernel_bytes(cfg, S, g)
+        kb = kernel_bytes(cfg, S, g, prof_n)
         ach = kb[dom] / (dom_ms * 1e-3) / 1e9
         line = {
             "metric": "timesteps/s", "value": value, "unit": "timesteps/s", "n_gpus": world, "steps": args.steps,
@@ -286,6 +287,7 @@ def main():
             "roofline": {"bound": "hbm", "kernel": dom, "achieved": ach, "peak": peak, "unit": "GB/s",
                          "frac": ach / peak, "traffic": ncu_traffic(dom), "peak_source": peak_src,
                          "algorithmic_bytes_per_launch": kb[dom], "launch_ms": dom_ms,
+                         "timesteps_per_launch": prof_n if dom == "k_fused2d" else 1,
                          "kernel_ms": {k: v[0] for k, v in prof.items() if v[1] > 0},
                          "kernel_share": {k: shares[k] / sum(shares.values()) for k in shares}},
             "roofline_step": {"B_alg_bytes": b_alg, "B_model_bytes": b_model,
@@ -303,8 +305,9 @@ def main():
         dist.destroy_process_group()
 
 
-def kernel_bytes(cfg, S, g):
-    """algorithmic bytes per launch of each kernel family (pruned count, SURVEY.md 8(d) / DESIGN.md)."""
+def kernel_bytes(cfg, S, g, steps_per_fused_launch):
+    """algorithmic bytes per launch of each kernel family (pruned count, SURVEY.md 8(d) / DESIGN.md).
+    k_fused2d runs every step of a pss_step(n) call in ONE launch: its bytes per launch are n * B_alg."""
     total = g.model_bytes_per_step(True)
     ndim = len(cfg["n"])
     model = cfg["model"]
@@ -319,7 +322,7 @@ def kernel_bytes(cfg, S, g):
     mid = 0.0
     if ndim == 3:
         mid = (total - rows - upd) / 2.0  # two k_mid launches per step (forward on groups, inverse on factors)
-    return {"k_rows": rows, "k_update": upd, "k_mid": mid}
+    return {"k_rows": rows, "k_update": upd, "k_mid": mid, "k_fused2d": total * steps_per_fused_launch}
 
 
 def ncu_traffic(kernel):

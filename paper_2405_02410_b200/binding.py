@@ -20,7 +20,7 @@ OK, EINVAL, EUNSUPPORTED, ESTATE, ECUDA = 0, -1, -2, -3, -4
 
 SYMBOLS = ["pss_create", "pss_add_field", "pss_add_linear", "pss_add_aux_def", "pss_add_term",
            "pss_set_noise", "pss_set_dealias", "pss_finalize", "pss_bind", "pss_set_field", "pss_step",
-           "pss_get_field", "pss_get_field_fourier", "pss_debug_noise", "pss_profile_step", "pss_launch_count",
+           "pss_get_field", "pss_get_field_fourier", "pss_debug_noise", "pss_profile_step", "pss_uses_fused_kernel", "pss_launch_count",
            "pss_model_bytes_per_step", "pss_step_count", "pss_strerror", "pss_last_cuda_error",
            "pss_destroy"]
 
@@ -68,6 +68,7 @@ def lib():
         L.pss_get_field_fourier.argtypes = [P, C.c_int, P, C.c_int]
         L.pss_debug_noise.argtypes = [P, C.c_int, C.c_uint64, P, P]
         L.pss_profile_step.argtypes = [P, C.c_int64, C.POINTER(C.c_double), C.POINTER(C.c_int64)]
+        L.pss_uses_fused_kernel.argtypes = [P]
         L.pss_launch_count.argtypes = [P]
         L.pss_launch_count.restype = C.c_uint64
         L.pss_model_bytes_per_step.argtypes = [P, C.c_int]
@@ -217,10 +218,14 @@ class System:
 
     def profile_step(self, n):
         """n steps with a CUDA-event pair around every launch -> {kernel: (mean ms per launch, launches)}."""
-        ms = (C.c_double * 3)()
-        cnt = (C.c_int64 * 3)()
+        ms = (C.c_double * 4)()
+        cnt = (C.c_int64 * 4)()
         self._chk(lib().pss_profile_step(self._h, int(n), ms, cnt))
-        return {k: (ms[i], int(cnt[i])) for i, k in enumerate(("k_rows", "k_update", "k_mid"))}
+        return {k: (ms[i], int(cnt[i])) for i, k in enumerate(("k_rows", "k_update", "k_mid", "k_fused2d"))}
+
+    @property
+    def uses_fused_kernel(self):
+        return bool(lib().pss_uses_fused_kernel(self._h))
 
     def synchronize(self):
         self._torch_stream.synchronize()

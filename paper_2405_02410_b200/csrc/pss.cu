@@ -16,6 +16,7 @@
 #include <vector>
 
 #include "pss_kernels.cuh"
+#include "pss_fused2d.cuh"
 
 namespace {
 
@@ -38,6 +39,8 @@ struct Plan {
   int mid_W, mid_threads; size_t mid_smem;
   int one_threads; size_t one_smem; /* 1D */
   int kx_keep_max;                  /* max over factors of the number of kept kx */
+  int fused;                        /* 1: the persistent 1024^2 fp32 kernel of pss_fused2d.cuh runs the steps */
+  int fused_prune;                  /* its input-pruned instantiation (mask cutoff <= n/4 on both axes)       */
 };
 
 }  // namespace
@@ -60,7 +63,8 @@ struct pss_system {
   size_t csize, rsize;
   int64_t M, N; /* modes (half-spectrum), sites */
   /* workspace carve-up (byte offsets) */
-  size_t off_state, off_psix, off_phat, off_scratch, off_ureal, off_tw[3], ws_need;
+  size_t off_state, off_psix, off_phat, off_scratch, off_ureal, off_tw[3], off_bar, ws_need;
+  unsigned long long bar_count; /* value of the fused kernel's grid-barrier counter */
   char *ws;
   cudaStream_t stream;
   std::string cuda_msg;
@@ -319,6 +323,20 @@ int round_threads(long long work) {
   return (int)t;
 }
 
+/* the persistent kernel of pss_fused2d.cuh: one real-coefficient field with one product group on 1024^2 fp32 */
+bool real_op(const DOp &d) { return ((d.a[0] + d.a[1] + d.a[2]) & 1) == 0; }
+bool fused2d_eligible(const pss_system *s) {
+  const Program &P = s->P;
+  if (env_int("PSS_FUSED", 1) == 0) return false;
+  if (s->ndim != 2 || s->prec != PSS_F32 || s->n[0] != f2d::N || s->n[1] != f2d::N) return false;
+  if (P.ndyn != 1 || P.nfac != 1 || P.ngrp != 1) return false;
+  if (P.dyn[0].lin_beg != P.dyn[0].lin_end) return false;
+  if (!real_op(P.grp[0].outer)) return false;
+  for (int e = P.dyn[0].lhs_beg; e < P.dyn[0].lhs_end; ++e) if (!real_op(P.lin[e])) return false;
+  for (int e = P.fac[0].lin_beg; e < P.fac[0].lin_end; ++e) if (!real_op(P.lin[e])) return false;
+  return true;
+}
+
 int make_plan(pss_system *s) {
   Plan &pl = s->plan;
   std::memset(&pl, 0, sizeof(pl));
@@ -335,6 +353,11 @@ int make_plan(pss_system *s) {
       if (cut > nxh) cut = nxh;
     }
     if (cut > pl.kx_keep_max) pl.kx_keep_max = cut;
+  }
+  pl.fused = fused2d_eligible(s) ? 1 : 0;
+  if (pl.fused) {
+    const int nn = (P.dealias == PSS_DEALIAS_OFF) ? 1 : ((P.dealias == PSS_DEALIAS_TWO_THIRDS ? 2 : P.fac[0].order) + 1);
+    pl.fused_prune = (nn >= 4) ? 1 : 0;
   }
   if (s->ndim == 1) {
     const size_t bufs = (size_t)(P.nfac + P.ngrp);
@@ -413,6 +436,7 @@ void carve_workspace(pss_system *s) {
   s->off_scratch = off; off += arr;
   s->off_ureal = off; off += align_up((size_t)s->N * s->rsize, 256);
   for (int j = 0; j < 3; ++j) { s->off_tw[j] = off; off += align_up((size_t)s->n[j] * s->csize, 256); }
+  s->off_bar = off; off += 256;
   s->ws_need = off;
 }
 
@@ -440,6 +464,24 @@ template <typename T> int set_attrs(pss_system *s) {
   return PSS_OK;
 }
 
+/* the persistent kernel needs every CTA co-resident (its phases are separated by a grid barrier): check that a
+ * cooperative launch of f2d::NCTA CTAs fits this device, else fall back to the two-kernel path. */
+int setup_fused(pss_system *s) {
+  if (!s->plan.fused) return PSS_OK;
+  int dev = 0, coop = 0, nsm = 0, occ = 0;
+  CK(cudaGetDevice(&dev));
+  CK(cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev));
+  CK(cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev));
+  CK(cudaFuncSetAttribute(f2d::k_fused2d<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)f2d::SMEM_BYTES));
+  CK(cudaFuncSetAttribute(f2d::k_fused2d<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)f2d::SMEM_BYTES));
+  if (s->plan.fused_prune)
+    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, f2d::k_fused2d<true>, f2d::THREADS, f2d::SMEM_BYTES));
+  else
+    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, f2d::k_fused2d<false>, f2d::THREADS, f2d::SMEM_BYTES));
+  if (!coop || (long long)occ * nsm < f2d::NCTA) s->plan.fused = 0;
+  return PSS_OK;
+}
+
 template <typename T> int upload_twiddles(pss_system *s) {
   typedef typename cplx_of<T>::type C;
   for (int j = 0; j < s->ndim; ++j) {
@@ -457,7 +499,7 @@ template <typename T> int upload_twiddles(pss_system *s) {
 }
 
 /* ---- launches -------------------------------------------------------------------------- */
-enum { KIND_ROWS = 0, KIND_UPDATE = 1, KIND_MID = 2 };
+enum { KIND_ROWS = 0, KIND_UPDATE = 1, KIND_MID = 2, KIND_FUSED = 3, KIND_COUNT = 4 };
 void prof_mark(pss_system *s, int kind, bool begin) {
   if (!s->prof_on) return;
   cudaEvent_t e;
@@ -531,6 +573,31 @@ template <typename T> int launch_rows(pss_system *s) {
   return PSS_OK;
 }
 
+/* nsteps steps (plus the E-rebuilding prologue when the state was just set) in one cooperative launch */
+int launch_fused(pss_system *s, int64_t nsteps) {
+  f2d::Args a;
+  a.state = carr<float>(s, s->off_state, 0);
+  a.E = carr<float>(s, s->off_psix, 0);
+  a.Z = carr<float>(s, s->off_phat, 0);
+  a.tw = twp<float>(s, 0);
+  a.bar = reinterpret_cast<unsigned long long *>(s->ws + s->off_bar);
+  a.bar_base = s->bar_count;
+  a.nsteps = nsteps;
+  a.step0 = s->step;
+  a.prologue = s->psix_valid ? 0 : 1;
+  void *params[2] = {(void *)&s->P, (void *)&a};
+  const void *fn = s->plan.fused_prune ? (const void *)f2d::k_fused2d<true> : (const void *)f2d::k_fused2d<false>;
+  prof_mark(s, KIND_FUSED, true);
+  cudaError_t e = cudaLaunchCooperativeKernel(fn, dim3(f2d::NCTA), dim3(f2d::THREADS), params, f2d::SMEM_BYTES, s->stream);
+  prof_mark(s, KIND_FUSED, false);
+  if (e != cudaSuccess) return cuda_fail(s, e, "k_fused2d");
+  CKL("k_fused2d");
+  s->bar_count += (unsigned long long)f2d::NCTA * (unsigned long long)(2 * nsteps + a.prologue);
+  s->psix_valid = true;
+  s->step += (uint64_t)nsteps;
+  return PSS_OK;
+}
+
 template <typename T> int do_steps(pss_system *s, int64_t nsteps) {
   const Program &P = s->P;
   if (nsteps == 0) return PSS_OK;
@@ -549,6 +616,7 @@ template <typename T> int do_steps(pss_system *s, int64_t nsteps) {
     return PSS_OK;
   }
   int rc;
+  if (s->plan.fused) return launch_fused(s, nsteps);
   if (P.nfac > 0 && !s->psix_valid) {
     if ((rc = launch_update<T>(s, 1, s->step)) != PSS_OK) return rc;
     s->psix_valid = true;
@@ -806,6 +874,8 @@ int pss_bind(pss_system *s, void *device_workspace, size_t bytes, void *cuda_str
   if (rc != PSS_OK) return rc;
   rc = (s->prec == PSS_F32) ? upload_twiddles<float>(s) : upload_twiddles<double>(s);
   if (rc != PSS_OK) return rc;
+  if ((rc = setup_fused(s)) != PSS_OK) return rc;
+  s->bar_count = 0; /* the counter lives in the workspace, zeroed above */
   s->bound = true;
   s->psix_valid = false;
   return PSS_OK;
@@ -857,14 +927,18 @@ int pss_debug_noise(pss_system *s, int field, uint64_t step, uint32_t *bits, voi
                               : do_debug_noise<double>(s, field, step, bits, z);
 }
 
-int pss_profile_step(pss_system *s, int64_t nsteps, double ms_per_launch[3], int64_t launches[3]) {
+int pss_profile_step(pss_system *s, int64_t nsteps, double ms_per_launch[4], int64_t launches[4]) {
   if (!s || nsteps < 0 || nsteps > 4096 || !ms_per_launch || !launches) return PSS_EINVAL;
   if (!s->finalized || !s->bound) return PSS_ESTATE;
   if (s->cuda_bad) return PSS_ECUDA;
   if (s->ndim == 1) return PSS_EUNSUPPORTED;
   int rc = (s->prec == PSS_F32) ? do_steps<float>(s, 0) : do_steps<double>(s, 0);
   /* make sure the prologue (if any) is not inside the profiled region */
-  if (s->P.nfac > 0 && !s->psix_valid) {
+  if (s->plan.fused && !s->psix_valid) {
+    rc = launch_fused(s, 0);
+    if (rc != PSS_OK) return rc;
+  }
+  if (!s->plan.fused && s->P.nfac > 0 && !s->psix_valid) {
     rc = (s->prec == PSS_F32) ? launch_update<float>(s, 1, s->step) : launch_update<double>(s, 1, s->step);
     if (rc != PSS_OK) return rc;
     s->psix_valid = true;
@@ -873,8 +947,8 @@ int pss_profile_step(pss_system *s, int64_t nsteps, double ms_per_launch[3], int
   rc = (s->prec == PSS_F32) ? do_steps<float>(s, nsteps) : do_steps<double>(s, nsteps);
   s->prof_on = false;
   cudaError_t e = cudaStreamSynchronize(s->stream);
-  double sum[3] = {0, 0, 0};
-  int64_t cnt[3] = {0, 0, 0};
+  double sum[KIND_COUNT] = {0, 0, 0, 0};
+  int64_t cnt[KIND_COUNT] = {0, 0, 0, 0};
   for (size_t i = 0; i < s->prof_kind.size() && 2 * i + 1 < s->prof_ev.size(); ++i) {
     float ms = 0.f;
     if (e == cudaSuccess && cudaEventElapsedTime(&ms, s->prof_ev[2 * i], s->prof_ev[2 * i + 1]) == cudaSuccess) {
@@ -885,12 +959,14 @@ int pss_profile_step(pss_system *s, int64_t nsteps, double ms_per_launch[3], int
   for (cudaEvent_t ev : s->prof_ev) cudaEventDestroy(ev);
   s->prof_ev.clear();
   s->prof_kind.clear();
-  for (int k = 0; k < 3; ++k) { ms_per_launch[k] = cnt[k] ? sum[k] / (double)cnt[k] : 0.0; launches[k] = cnt[k]; }
+  for (int k = 0; k < KIND_COUNT; ++k) { ms_per_launch[k] = cnt[k] ? sum[k] / (double)cnt[k] : 0.0; launches[k] = cnt[k]; }
   if (e != cudaSuccess) return cuda_fail(s, e, "pss_profile_step");
   return rc;
 }
 
 uint64_t pss_launch_count(const pss_system *s) { return s ? s->launches : 0; }
+
+int pss_uses_fused_kernel(const pss_system *s) { return (s && s->finalized && s->bound && s->plan.fused) ? 1 : 0; }
 
 double pss_model_bytes_per_step(const pss_system *s, int pruned) {
   if (!s || !s->finalized) return 0.0;
