@@ -44,9 +44,9 @@ constexpr int N = 1024;          /* lattice points per axis          */
 constexpr int NP = 512;          /* packed row pairs (p, p+512)      */
 constexpr int PITCH = 33;        /* exchange row pitch (complex)     */
 constexpr int XBUF = 32 * PITCH + 8; /* one exchange region; +64 B so that neighbouring regions differ by 16 banks */
-constexpr int THREADS = 128;
+constexpr int THREADS = 256;     /* warps 0-3 transform, warps 4-7 draw the next step's noise concurrently */
 constexpr int NCTA = 129;        /* 128 CTAs own 4 packed rows and 4 columns each; CTA 128 owns column kx = 512 */
-constexpr size_t SMEM_BYTES = (size_t)(N + 2 * 4 * XBUF + 4 * N) * sizeof(float2) + (size_t)4 * N * sizeof(float4);
+constexpr size_t SMEM_BYTES = (size_t)(N + 2 * 4 * XBUF + 2 * 4 * N) * sizeof(float2) + (size_t)4 * N * sizeof(float4);
 
 struct Args {
   float2 *state;
@@ -117,10 +117,13 @@ __device__ __forceinline__ void fft32(float2 (&v)[32]) {
   }
 }
 
+/* the four transform warps only (named barrier 1) */
+__device__ __forceinline__ void fft_warps_sync() { asm volatile("bar.sync 1, 128;" ::: "memory"); }
+
 /* one 1024-point forward transform of the line this thread group holds: thread `me` (0..31) enters with
  * v[n1] = x[32 n1 + me] and leaves with X[me + 32 k2] at v[brev5(k2)].  Two radix-32 passes around one
  * shared-memory exchange; tws[a*32+b] = exp(-2 pi i a b / 1024).  `cta_sync`: the 32 threads of the line
- * sit in different warps (phase R) -> __syncthreads, else (phase C, one warp per line) __syncwarp. */
+ * sit in different warps (phase R) -> barrier over the four transform warps, else (phase C, one warp per line) __syncwarp. */
 __device__ __forceinline__ void fft1024(float2 (&v)[32], float2 *xs, const float2 *tws, int me, bool cta_sync) {
 #pragma unroll 1
   for (int h = 0; h < 2; ++h) {
@@ -135,21 +138,110 @@ __device__ __forceinline__ void fft1024(float2 (&v)[32], float2 *xs, const float
         }
         xs[i * PITCH + me] = x;
       }
-      if (cta_sync) __syncthreads(); else __syncwarp();
+      if (cta_sync) fft_warps_sync(); else __syncwarp();
 #pragma unroll
       for (int i = 0; i < 32; ++i) v[i] = xs[me * PITCH + i];
     }
   }
 }
 
-__device__ __forceinline__ unsigned long long ld_acquire_u64(const unsigned long long *p) {
+/* ---- noise (Eq. 16): Philox4x32-10 + Box-Muller, the same stream as noise_z() of
+ * pss_pointwise.cuh (same counter, same words, same uniforms) with leaner arithmetic: 32-bit mode index,
+ * step-invariant half of round 1 left to the compiler to hoist, and own fp32 ln / sin / cos kernels
+ * (coefficients fitted for this file; each within ~1 ulp of the exact value over all 2^24 inputs). ---- */
+struct NoiseKey {
+  uint32_t c2, c3;   /* counter words 2, 3: step_lo, ((step_hi & 0xffff) << 16) | field */
+  uint32_t k0, k1;   /* key = seed */
+};
+
+__device__ __forceinline__ void philox_w01(uint32_t c0, const NoiseKey &K, uint32_t &w0, uint32_t &w1) {
+  uint32_t c1 = 0u, c2 = K.c2, c3 = K.c3, k0 = K.k0, k1 = K.k1;
+#pragma unroll
+  for (int r = 0; r < 10; ++r) {
+    const uint32_t hi0 = __umulhi(0xD2511F53u, c0), lo0 = 0xD2511F53u * c0;
+    const uint32_t hi1 = __umulhi(0xCD9E8D57u, c2), lo1 = 0xCD9E8D57u * c2;
+    const uint32_t n0 = hi1 ^ c1 ^ k0, n2 = hi0 ^ c3 ^ k1;
+    c0 = n0; c1 = lo1; c2 = n2; c3 = lo0;
+    k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
+  }
+  w0 = c0; w1 = c1;
+}
+
+/* sqrt(-ln u1) * (cos 2 pi u2, sin 2 pi u2) with u1 = ((w0>>8)+1) 2^-24 in (0,1], u2 = (w1>>8) 2^-24 in [0,1):
+ * this is (g1 + i g2)/sqrt(2) of the Box-Muller pair g = sqrt(-2 ln u1) (cos, sin). */
+__device__ __forceinline__ float2 box_muller_half(uint32_t w0, uint32_t w1) {
+  /* ln u1: u1 = m 2^e, m in [2/3, 4/3); ln m = f - f^2/2 + f^3 P(f), f = m - 1 */
+  const float u1 = (float)((w0 >> 8) + 1u) * (1.0f / 16777216.0f);
+  const int iu = __float_as_int(u1);
+  const int e = (iu - 0x3f2aaaab) & 0xff800000;
+  const float f = __int_as_float(iu - e) - 1.0f;
+  const float fe = (float)e * 1.1920928955078125e-07f;
+  float p = -0.12429866194725037f;
+  p = fmaf(p, f, 0.13433773815631866f);
+  p = fmaf(p, f, -0.12287236750125885f);
+  p = fmaf(p, f, 0.14116978645324707f);
+  p = fmaf(p, f, -0.166733980178833f);
+  p = fmaf(p, f, 0.2000383585691452f);
+  p = fmaf(p, f, -0.24999943375587463f);
+  p = fmaf(p, f, 0.33333319425582886f);
+  const float f2 = f * f;
+  const float lnm = fmaf(p * f, f2, -0.5f * f2) + f;
+  const float x = -fmaf(fe, 0.693147182464599609375f, lnm);          /* -ln u1 >= 0 */
+  /* sqrt by rsqrt + one Newton step; x = 0 (u1 = 1) gives 0 */
+  const float y = rsqrtf(fmaxf(x, 1e-30f));
+  float r = x * y;
+  r = fmaf(0.5f * y, fmaf(-r, r, x), r);
+  /* angle 2 pi j / 2^24: nearest quadrant q, remainder phi in [-pi/4, pi/4) exactly representable */
+  const uint32_t j = w1 >> 8;
+  const uint32_t qq = (j + (1u << 21)) >> 22;
+  const int rem = (int)j - (int)(qq << 22);
+  const float phi = (float)rem * 3.7450702829191576e-07f;             /* 2 pi / 2^24 */
+  const float u = phi * phi;
+  float sp = 2.7249941467744065e-06f, cp = -4.133496076974552e-06f;
+  sp = fmaf(sp, u, -0.00019840087043121457f);
+  cp = fmaf(cp, u, 2.896795376727823e-05f);
+  sp = fmaf(sp, u, 0.008333331905305386f);
+  cp = fmaf(cp, u, -0.0013901740312576294f);
+  sp = fmaf(sp, u, -0.1666666716337204f);
+  cp = fmaf(cp, u, 0.04166676476597786f);
+  const float sn = fmaf(phi * u, sp, phi);
+  const float cn = fmaf(u * u, cp, fmaf(-0.5f, u, 1.0f));
+  const float ca = (qq & 1u) ? sn : cn, sa = (qq & 1u) ? cn : sn;     /* |cos|, |sin| carriers */
+  const float c = ((qq + 1u) & 2u) ? -ca : ca;                        /* q = 1, 2 -> negative cosine */
+  const float sgn = (qq & 2u) ? -sa : sa;                             /* q = 2, 3 -> negative sine   */
+  return make_float2(r * c, r * sgn);
+}
+
+/* unit Hermitian complex Gaussian of logical mode (kx, ky) on the 1024 x 513 half-spectrum; `plane`: kx is 0 or 512 */
+__device__ __forceinline__ float2 noise_mode(const NoiseKey &K, int kx, int ky, bool plane) {
+  uint32_t m = (uint32_t)(ky * (N / 2 + 1) + kx);
+  bool self = false, other = false;
+  if (plane) {
+    const int kyp = (N - ky) & (N - 1);
+    const uint32_t mp = (uint32_t)(kyp * (N / 2 + 1) + kx);
+    self = (mp == m);
+    other = (mp < m);
+    m = other ? mp : m;
+  }
+  uint32_t w0, w1;
+  philox_w01(m, K, w0, w1);
+  float2 z = box_muller_half(w0, w1);
+  if (plane) {
+    if (self) z = make_float2(z.x * 1.41421356237309504880f, 0.f);
+    else if (other) z.y = -z.y;
+  }
+  return z;
+}
+
+__device__ __forceinline__ unsigned long long ld_relaxed_u64(const unsigned long long *p) {
   unsigned long long v;
-  asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+  asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
   return v;
 }
 
-/* grid barrier over all CTAs of the (cooperative, co-resident) grid, split in two so that independent work
- * (the next noise draw) can run between arriving and waiting.  `target` = counter value once all arrived. */
+/* grid barrier over all CTAs of the (cooperative, co-resident) grid, split in two.  `target` = counter value
+ * once all arrived.  Data crossing the barrier is written with plain stores (made visible by the fence before
+ * the arrival) and read with ld.global.cg, so the L1 never has to be invalidated while polling. */
 __device__ __forceinline__ void grid_arrive(unsigned long long *ctr) {
   __syncthreads();
   if (threadIdx.x == 0) {
@@ -159,24 +251,25 @@ __device__ __forceinline__ void grid_arrive(unsigned long long *ctr) {
 }
 __device__ __forceinline__ void grid_wait(const unsigned long long *ctr, unsigned long long target) {
   if (threadIdx.x == 0) {
-    while (ld_acquire_u64(ctr) < target) { }
+    while (ld_relaxed_u64(ctr) < target) { }
+    __threadfence();
   }
   __syncthreads();
 }
-
 /* ------------------------------------------------------------------------------------------ */
 template <bool PRUNE>
 __global__ void __launch_bounds__(THREADS, 1) k_fused2d(const __grid_constant__ Program P, const Args A) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  float2 *tws = reinterpret_cast<float2 *>(smem_raw);          /* [32][32]                       */
-  float2 *xa = tws + N;                                        /* [4][XBUF] exchange, inverse    */
-  float2 *xb = xa + 4 * XBUF;                                  /* [4][XBUF] exchange, forward    */
-  float2 *zbuf = xb + 4 * XBUF;                                /* [4][32 k2][32 k1] noise z      */
-  float4 *tab = reinterpret_cast<float4 *>(zbuf + 4 * N);      /* [4][32 k2][32 k1] coefficients */
+  float2 *tws = reinterpret_cast<float2 *>(smem_raw);          /* [32][32]                          */
+  float2 *xa = tws + N;                                        /* [4][XBUF] exchange, inverse       */
+  float2 *xb = xa + 4 * XBUF;                                  /* [4][XBUF] exchange, forward       */
+  float2 *zbuf = xb + 4 * XBUF;                                /* [2][4][32 k2][32 k1] noise z      */
+  float4 *tab = reinterpret_cast<float4 *>(zbuf + 2 * 4 * N);  /* [4][32 k2][32 k1] coefficients    */
 
-  const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
+  const int tid = threadIdx.x, lane = tid & 31, w = (tid >> 5) & 3;
+  const bool noisew = tid >= 128;
   const int b = blockIdx.x;
-  /* phase C ownership: one column per warp */
+  /* phase C ownership: one column per transform warp (and per noise warp) */
   int kx;
   if (b < 128) kx = (w < 2) ? (2 * b + w) : (256 + 2 * b + (w - 2));
   else kx = (w == 0) ? 512 : -1;
@@ -184,17 +277,63 @@ __global__ void __launch_bounds__(THREADS, 1) k_fused2d(const __grid_constant__ 
   const int kxm = colw ? ((N - kx) & (N - 1)) : 0;
   const bool selfc = (kx == 0) || (kx == 512);
   const DDyn &D0 = P.dyn[0];
+  const long long nphase = A.nsteps + (A.prologue ? 1 : 0);
+  unsigned long long bar_target = A.bar_base;
+
+  if (noisew) {
+    /* ================= noise warps: z(step + 1) while the transform warps work on `step` ================= */
+    const bool draw = colw && D0.noisy;
+    NoiseKey K;
+    K.k0 = P.seed_lo;
+    K.k1 = P.seed_hi;
+    float2 *zw = zbuf + (size_t)w * N + lane;
+    if (draw && A.nsteps > 0) {
+      K.c2 = (uint32_t)(A.step0 & 0xffffffffu);
+      K.c3 = (uint32_t)((((A.step0 >> 32) & 0xffffu) << 16) | ((uint32_t)D0.field_id & 0xffffu));
+#pragma unroll 2
+      for (int k2 = 0; k2 < 32; ++k2) zw[k2 * 32] = noise_mode(K, kx, lane + 32 * k2, selfc);
+    }
+    __syncthreads();
+#pragma unroll 1
+    for (long long it = 0; it < nphase; ++it) {
+      const bool pro = A.prologue && it == 0;
+      const long long ls = it - (A.prologue ? 1 : 0);
+      const bool more = draw && !pro && (ls + 1 < A.nsteps);
+      const unsigned long long nstep = A.step0 + (unsigned long long)(ls + 1);
+      K.c2 = (uint32_t)(nstep & 0xffffffffu);
+      K.c3 = (uint32_t)((((nstep >> 32) & 0xffffu) << 16) | ((uint32_t)D0.field_id & 0xffffu));
+      float2 *zn = zw + (size_t)((ls + 1) & 1) * 4 * N;
+      if (!pro) {
+        if (more) {
+#pragma unroll 2
+          for (int k2 = 0; k2 < 16; ++k2) zn[k2 * 32] = noise_mode(K, kx, lane + 32 * k2, selfc);
+        }
+        grid_arrive(A.bar);
+        bar_target += NCTA;
+        grid_wait(A.bar, bar_target);
+        if (more) {
+#pragma unroll 2
+          for (int k2 = 16; k2 < 32; ++k2) zn[k2 * 32] = noise_mode(K, kx, lane + 32 * k2, selfc);
+        }
+      }
+      grid_arrive(A.bar);
+      bar_target += NCTA;
+      grid_wait(A.bar, bar_target);
+    }
+    return;
+  }
+
+  /* ================= transform warps ================= */
   const bool need_inv = colw && keep_axis(P.dealias, P.fac[0].order, kx, N);
   /* phase R ownership: thread = (packed row pl of this CTA, butterfly slot) */
   const int s8 = lane & 7, pl = lane >> 3, slot = 8 * w + s8;
   const bool roww = b < 128;
 
-  for (int i = tid; i < N; i += THREADS) tws[i] = A.tw[((i >> 5) * (i & 31)) & (N - 1)];
+  for (int i = tid; i < N; i += 128) tws[i] = A.tw[((i >> 5) * (i & 31)) & (N - 1)];
 
   /* per-mode coefficients of this warp's column: (dt*outer, 1/(1 - dt L), noise amplitude, factor op * mask / N) */
   float2 st[32];
   float4 *mytab = tab + (size_t)w * N;
-  float2 *myz = zbuf + (size_t)w * N;
   if (colw) {
     const float dt = (float)P.dt, invN = (float)P.invN;
     const bool keepx = keep_axis(P.dealias, P.fac[0].order, kx, N);
@@ -215,7 +354,10 @@ __global__ void __launch_bounds__(THREADS, 1) k_fused2d(const __grid_constant__ 
       }
       t.w = fc;
       mytab[k2 * 32 + lane] = t;
-      myz[k2 * 32 + lane] = make_float2(0.f, 0.f);
+      if (!D0.noisy) {
+        zbuf[(size_t)w * N + k2 * 32 + lane] = make_float2(0.f, 0.f);
+        zbuf[(size_t)(4 + w) * N + k2 * 32 + lane] = make_float2(0.f, 0.f);
+      }
     }
 #pragma unroll
     for (int k2 = 0; k2 < 32; ++k2) st[k2] = A.state[(size_t)kx * N + lane + 32 * k2];
@@ -231,13 +373,12 @@ __global__ void __launch_bounds__(THREADS, 1) k_fused2d(const __grid_constant__ 
   }
   __syncthreads();
 
-  unsigned long long bar_target = A.bar_base;
-  const long long nphase = A.nsteps + (A.prologue ? 1 : 0);
   float2 v[32];
 #pragma unroll 1
   for (long long it = 0; it < nphase; ++it) {
     const bool pro = A.prologue && it == 0;
-    const unsigned long long step = A.step0 + (unsigned long long)(it - (A.prologue ? 1 : 0));
+    const long long ls = it - (A.prologue ? 1 : 0);
+    const float2 *myz = zbuf + (size_t)(ls & 1) * 4 * N + (size_t)w * N + lane;
     if (pro && need_inv) {
 #pragma unroll
       for (int k2 = 0; k2 < 32; ++k2) {
@@ -296,7 +437,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_fused2d(const __grid_constant__ 
 #pragma unroll
           for (int k2 = 0; k2 < 32; ++k2) {
             const float4 tt = mytab[k2 * 32 + lane];
-            const float2 z = myz[k2 * 32 + lane];
+            const float2 z = myz[k2 * 32];
             const float2 pq = v[brev5(k2)];
             const float nx = (st[k2].x + tt.x * pq.x) + tt.z * z.x;
             const float ny = (st[k2].y + tt.x * pq.y) + tt.z * z.y;
@@ -322,18 +463,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_fused2d(const __grid_constant__ 
           }
         }
       }
-      if (t == 1) {
-        /* between arriving and waiting: this step's noise for the warp's own column (Eq. 16) */
-        grid_arrive(A.bar);
-        if (colw && D0.noisy) {
-#pragma unroll 1
-          for (int k2 = 0; k2 < 32; ++k2)
-            myz[k2 * 32 + lane] = noise_z<float>(P, D0.field_id, step, kx, lane + 32 * k2, 0);
-          __syncwarp();
-        }
-        bar_target += NCTA;
-        grid_wait(A.bar, bar_target);
-      } else if (t == 3) {
+      if (t == 1 || t == 3) {
         grid_arrive(A.bar);
         bar_target += NCTA;
         grid_wait(A.bar, bar_target);
