@@ -31,7 +31,7 @@ if ROOT not in sys.path:
 
 import numpy as np  # noqa: E402
 
-from paper_2405_02410_b200 import workloads as wl  # noqa: E402
+from paper_2405_02410_b200 import replicas, workloads as wl  # noqa: E402
 
 FALLBACK_HBM_GBS = 6650.0  # /opt/skills/guides/B200_PROFILING.md "FALLBACK"
 
@@ -172,8 +172,7 @@ def main():
     import paper_2405_02410_b200 as pss
 
     # replicas only: every rank advances its own realisation (seed + rank), no data-path collective
-    cfg_r = dict(cfg)
-    cfg_r["seed"] = cfg["seed"] + rank
+    cfg_r = replicas.rank_config(cfg, rank)
     g, ids = wl.build(pss, cfg_r, prec=args.prec, device="cuda:%d" % local_rank)
     dyn_names = list(cfg["ic"].keys())
     sites = int(np.prod(cfg["n"]))
@@ -248,11 +247,7 @@ def main():
     barrier()
 
     # max over ranks of the timed totals; sum of units
-    t_total = torch.tensor([total_ms, e2e_s], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t_total, op=dist.ReduceOp.MAX)
-    total_ms, e2e_s = float(t_total[0]), float(t_total[1])
-    steps_all = world * args.steps * inner
+    (total_ms, e2e_s), steps_all = replicas.reduce_timings([total_ms, e2e_s], args.steps * inner, device=dev)
     value = steps_all / (total_ms * 1e-3)
     e2e_value = world * e2e_steps * inner / e2e_s
 

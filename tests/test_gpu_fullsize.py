@@ -1,0 +1,135 @@
+"""GPU parity at BASELINE.json's FULL sizes, in the launch configuration bench.py times (one pss_step(n)
+call per run of n steps), against the CPU oracle on the same seeded inputs and the same noise stream.
+
+Tolerances: north_star — relative L2 <= 1e-5 after 1 step, <= 1e-3 after 1000 steps (fp32);
+<= 1e-12 / 1e-9 (fp64).  Config 4 (nematic): 250-step horizon, reading A20 of DESIGN.md.
+Intermediate horizons (10-20 steps) use 10x the 1-step tolerance.
+"""
+import numpy as np
+import pytest
+
+from paper_2405_02410_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+TOL1 = {"f32": 1e-5, "f64": 1e-12}
+TOLN = {"f32": 1e-3, "f64": 1e-9}
+
+
+@pytest.fixture(scope="module")
+def pss():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    import paper_2405_02410_b200 as p
+    p.binding.lib()
+    return p
+
+
+def rel_l2(a, b):
+    a = np.asarray(a, dtype=np.float64)
+    b = np.asarray(b, dtype=np.float64)
+    den = np.linalg.norm(b.ravel())
+    return np.linalg.norm((a - b).ravel()) / (den if den > 0 else 1.0)
+
+
+def both(pss, oracle, cfg, prec):
+    g, ids = wl.build(pss, cfg, prec=prec)
+    o, ids_o = wl.build(oracle, cfg, prec=prec)
+    assert ids == ids_o
+    return g, o, [ids[name] for name in cfg["ic"].keys()]
+
+
+def check(g, o, dyn, tol, what):
+    worst = 0.0
+    for f in dyn:
+        a, b = g.get_field(f), o.get_field(f)
+        assert np.all(np.isfinite(a)), what
+        e = rel_l2(a, b)
+        worst = max(worst, e)
+        assert e <= tol, "%s: field %d rel L2 %.3e > %.1e" % (what, f, e, tol)
+    print("%s: rel L2 %.3e (tol %.1e)" % (what, worst, tol))
+    return worst
+
+
+def run_horizons(pss, oracle, cfg, prec, horizons, what):
+    """horizons: [(total steps, tolerance), ...] increasing; each increment is ONE pss_step(n) call."""
+    g, o, dyn = both(pss, oracle, cfg, prec)
+    done = 0
+    for total, tol in horizons:
+        g.step(total - done)
+        o.step(total - done)
+        done = total
+        assert g.step_count == total
+        check(g, o, dyn, tol, "%s %s, %d steps" % (what, prec, total))
+    return g
+
+
+# config 2: 2D Model B 1024^2, fp32 (the headline; persistent fused kernel) and fp64 (generic kernels)
+@pytest.mark.parametrize("prec", ["f32", "f64"])
+def test_config2_modelb_1024_1000_steps(pss, oracle, prec):
+    cfg = wl.make_config("modelb_1024")
+    g = run_horizons(pss, oracle, cfg, prec, [(1, TOL1[prec]), (1000, TOLN[prec])], "config 2 (1024^2)")
+    assert bool(g.uses_fused_kernel) == (prec == "f32"), "the headline config must run the kernel bench.py times"
+
+
+def test_config2_noise_bits_full_size(pss, oracle):
+    cfg = wl.make_config("modelb_1024")
+    g, o, dyn = both(pss, oracle, cfg, "f32")
+    for step in (0, 999):
+        bg, zg = g.debug_noise(dyn[0], step)
+        bo, zo = o.debug_noise(dyn[0], step)
+        assert np.array_equal(bg, bo)
+        assert np.max(np.abs(zg - zo)) <= 3e-6
+
+
+def test_config2_other_dealias_rules_full_size(pss, oracle):
+    """forced 2/3 rule (literal BASELINE wording, A6) and no mask: the un-pruned fused instantiation"""
+    for rule in (1, 2):
+        cfg = wl.make_config("modelb_1024")
+        g, ids = wl.build(pss, cfg, prec="f32", dealias=rule)
+        o, _ = wl.build(oracle, cfg, prec="f32", dealias=rule)
+        g.step(1)
+        o.step(1)
+        check(g, o, [ids["phi"]], TOL1["f32"], "config 2 dealias=%d, 1 step" % rule)
+        g.step(19)
+        o.step(19)
+        check(g, o, [ids["phi"]], 10 * TOL1["f32"], "config 2 dealias=%d, 20 steps" % rule)
+
+
+# config 3: 3D Model B 256^3 fp32
+def test_config3_modelb_256_cubed(pss, oracle):
+    cfg = wl.make_config("modelb_256c")
+    run_horizons(pss, oracle, cfg, "f32", [(1, TOL1["f32"]), (10, 10 * TOL1["f32"])], "config 3 (256^3)")
+
+
+# config 4: nematic 1024^2 fp32, parity horizon 250 steps (A20)
+def test_config4_nematic_1024(pss, oracle):
+    cfg = wl.make_config("nematic_1024")
+    run_horizons(pss, oracle, cfg, "f32", [(1, TOL1["f32"]), (250, 1e-3)], "config 4 (nematic 1024^2)")
+
+
+# config 5: KPZ 4096^2 fp32
+def test_config5_kpz_4096(pss, oracle):
+    cfg = wl.make_config("kpz_4096")
+    run_horizons(pss, oracle, cfg, "f32", [(1, TOL1["f32"]), (20, 10 * TOL1["f32"])], "config 5 (KPZ 4096^2)")
+
+
+# config 5b: the Model-B lattice sweep 256^2 .. 8192^2
+@pytest.mark.parametrize("n", [256, 512, 2048, 4096, 8192])
+def test_sweep_modelb(pss, oracle, n):
+    cfg = wl.make_config("sweep_%d" % n)
+    run_horizons(pss, oracle, cfg, "f32", [(1, TOL1["f32"]), (5, 10 * TOL1["f32"])], "sweep %d^2" % n)
+
+
+def test_fullsize_step_splitting_is_bit_identical(pss):
+    """pss_step(a); pss_step(b) == pss_step(a+b) bit for bit in the fused kernel (P14 at full size)"""
+    cfg = wl.make_config("modelb_1024")
+    a, ids = wl.build(pss, cfg, prec="f32")
+    b, _ = wl.build(pss, cfg, prec="f32")
+    a.step(3)
+    a.step(4)
+    b.step(7)
+    f = ids["phi"]
+    assert np.array_equal(a.get_field_fourier(f).view(np.uint32), b.get_field_fourier(f).view(np.uint32))
+    m = a.get_field_fourier(f)[0, 0]
+    assert m.imag == 0.0
