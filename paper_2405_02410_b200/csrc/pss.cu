@@ -438,7 +438,7 @@ void carve_workspace(pss_system *s) {
   s->off_scratch = off; off += arr;
   s->off_ureal = off; off += align_up((size_t)s->N * s->rsize, 256);
   for (int j = 0; j < 3; ++j) { s->off_tw[j] = off; off += align_up((size_t)s->n[j] * s->csize, 256); }
-  s->off_bar = off; off += 256;
+  s->off_bar = off; off += 1024; /* v1: one 64-bit counter; v2: one 32-bit epoch flag per CTA */
   s->ws_need = off;
 }
 
@@ -599,6 +599,7 @@ int launch_fused(pss_system *s, int64_t nsteps) {
   a.nsteps = nsteps;
   a.step0 = s->step;
   a.prologue = s->psix_valid ? 0 : 1;
+  a.dbg = env_int("PSS_DBG", 0);
   void *params[2] = {(void *)&s->P, (void *)&a};
   const bool v2 = s->plan.fused == 2;
   const void *fn = v2 ? (s->plan.fused_prune ? (const void *)f2e::k_fused2d_v2<true> : (const void *)f2e::k_fused2d_v2<false>)

@@ -58,6 +58,7 @@ struct Args {
   long long nsteps;
   unsigned long long step0;
   int prologue;                  /* 1: E is stale (after pss_set_field): rebuild it from the state first */
+  int dbg;                       /* timing experiments only (PSS_DBG): 1 no barrier wait, 2 no FFT, 4 no global ld/st, 8 no noise */
 };
 
 __device__ __forceinline__ float2 ldcg2(const float2 *p) { return __ldcg(p); }

@@ -138,14 +138,18 @@ __device__ __forceinline__ void fwd_dit(float2 (&v)[16], const Lane &ln) {
   dft_reg<4, -1>(v);
 }
 
-/* grid barrier over the transform threads of all CTAs (the noise warps never take part) */
-__device__ __forceinline__ void grid_barrier(unsigned long long *ctr, unsigned long long target) {
+/* grid barrier over the transform threads of all CTAs (the noise warps never take part): one monotonically
+ * increasing 64-bit counter.  Thread 0 arrives with a release reduction once the CTA's 256 threads have passed
+ * tsync (their data stores happen-before it through the CTA barrier) and polls with acquire loads; data crossing the
+ * barrier is read with ld.global.cg. */
+__device__ __forceinline__ void grid_barrier(unsigned long long *ctr, unsigned long long target, int dbg) {
   tsync();
   if (threadIdx.x == 0) {
-    __threadfence();
-    atomicAdd(ctr, 1ULL);
-    while (f2d::ld_relaxed_u64(ctr) < target) { }
-    __threadfence();
+    asm volatile("red.release.gpu.global.add.u64 [%0], 1;" ::"l"(ctr) : "memory");
+    if (!(dbg & 1)) {
+      unsigned long long v;
+      do { asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(ctr) : "memory"); } while (v < target);
+    }
   }
   tsync();
 }
@@ -189,7 +193,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_fused2d_v2(const __grid_constant
       K.c3 = (uint32_t)((((step >> 32) & 0xffffu) << 16) | ((uint32_t)D0.field_id & 0xffffu));
       const int buf = (int)(s & 1);
       if (s >= 2) nb_sync(4 + buf); /* the transform warps have consumed z(s-2) */
-      if (colw) {
+      if (colw && !(A.dbg & 8)) {
         float2 *zw = zbuf + (size_t)buf * 16 * TT + tid;
 #pragma unroll 2
         for (int r = 0; r < 16; ++r)
@@ -273,7 +277,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_fused2d_v2(const __grid_constant
 #pragma unroll 1
     for (int t = pro ? 3 : 0; t < 4; ++t) {
       if (t == 0) {
-        if (roww) {
+        if (roww && !(A.dbg & 4)) {
           const float2 *Eb = A.E + ((size_t)b * N) * 4 + L + (size_t)kyb * 4;
 #pragma unroll
           for (int r = 0; r < 16; ++r) {
@@ -286,7 +290,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_fused2d_v2(const __grid_constant
           }
         }
       } else if (t == 2) {
-        if (colw) {
+        if (colw && !(A.dbg & 4)) {
           const float2 *Z1 = A.Z + (size_t)kx * NP + tq, *Z2 = A.Z + (size_t)kxm * NP + tq;
 #pragma unroll
           for (int a = 0; a < 8; ++a) {
@@ -299,7 +303,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_fused2d_v2(const __grid_constant
           for (int a = 0; a < 16; ++a) v[a] = make_float2(0.f, 0.f);
         }
       }
-      if (t == 0 || t == 3) fwd_dit(v, ln); else fwd_dif(v, ln);
+      if (!(A.dbg & 2)) { if (t == 0 || t == 3) fwd_dit(v, ln); else fwd_dif(v, ln); }
       if (t == 0) {
         /* conj(v[a]) = a(x) + i b(x) at x = 64 a + tq: rows p and p + 512 in real space */
 #pragma unroll
@@ -309,13 +313,13 @@ __global__ void __launch_bounds__(THREADS, 1) k_fused2d_v2(const __grid_constant
         }
         tsync(); /* everybody has left fwd_dit's last exchange read before fwd_dif writes */
       } else if (t == 1) {
-        if (roww) {
+        if (roww && !(A.dbg & 4)) {
           float2 *Zb = A.Z + (size_t)kyb * NP + 4 * b + L;
 #pragma unroll
           for (int r = 0; r < 16; ++r) Zb[(size_t)(16 * (r & 3) + 256 * (r >> 2)) * NP] = v[r];
         }
         bar_target += NCTA;
-        grid_barrier(A.bar, bar_target);
+        grid_barrier(A.bar, bar_target, A.dbg);
       } else if (t == 2) {
         /* v[r] = P_q at ky(r): Eq. 15 + Eq. 16 + Eq. 18, then the next factor's (conjugated) input */
         if (noisy) nb_sync(2 + zb);
@@ -334,7 +338,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_fused2d_v2(const __grid_constant
         tsync();
       } else {
         /* conj(v[a]) = psi_x[kx][y = 64 a + tq]; pack rows y (A) and y + 512 (B) */
-        if (need_inv) {
+        if (need_inv && !(A.dbg & 4)) {
 #pragma unroll
           for (int a = 0; a < 8; ++a) {
             const float2 av = make_float2(v[a].x, -v[a].y);
@@ -350,7 +354,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_fused2d_v2(const __grid_constant
           }
         }
         bar_target += NCTA;
-        grid_barrier(A.bar, bar_target);
+        grid_barrier(A.bar, bar_target, A.dbg);
       }
     }
   }
