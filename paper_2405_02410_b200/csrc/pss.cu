@@ -65,7 +65,7 @@ struct pss_system {
   size_t csize, rsize;
   int64_t M, N; /* modes (half-spectrum), sites */
   /* workspace carve-up (byte offsets) */
-  size_t off_state, off_psix, off_phat, off_scratch, off_ureal, off_tw[3], off_bar, ws_need;
+  size_t off_state, off_psix, off_phat, off_scratch, off_ureal, off_tw[3], off_rev, off_bar, ws_need;
   unsigned long long bar_count; /* value of the fused kernel's grid-barrier counter */
   char *ws;
   cudaStream_t stream;
@@ -110,6 +110,11 @@ int cuda_fail(pss_system *s, cudaError_t e, const char *what) {
     if (e_ != cudaSuccess) return cuda_fail(s, e_, name);          \
     s->launches += 1;                                              \
   } while (0)
+
+int env_int(const char *name, int dflt) {
+  const char *v = std::getenv(name);
+  return (v && *v) ? std::atoi(v) : dflt;
+}
 
 /* ---- term-list compiler ---------------------------------------------------------------- */
 DOp link_op(const pss_system *s, const pss_op &op, int src_slot) {
@@ -295,6 +300,25 @@ int build_program(pss_system *s) {
   if (lin.size() > PSS_P_MAX_LIN) return PSS_EUNSUPPORTED;
   for (size_t i = 0; i < lin.size(); ++i) P.lin[i] = lin[i];
   P.nlin = (int32_t)lin.size();
+  /* radial fast path: all coefficients are polynomials in q^2 */
+  {
+    auto radial = [](const DOp &d) { return d.p == 0 && d.a[0] == 0 && d.a[1] == 0 && d.a[2] == 0 && d.zflags == 0 && d.m <= 4; };
+    bool ok = env_int("PSS_RADIAL", 1) != 0 && P.ndyn == 1 && P.ngrp <= 1 && P.nfac <= 1 &&
+              P.dyn[0].lin_beg == P.dyn[0].lin_end;
+    if (ok && P.dyn[0].noisy && (P.dyn[0].noise_qpow < 0 || (P.dyn[0].noise_qpow & 1))) ok = false;
+    for (int e = P.dyn[0].lhs_beg; ok && e < P.dyn[0].lhs_end; ++e) ok = radial(P.lin[e]);
+    if (ok && P.ngrp == 1) ok = radial(P.grp[0].outer);
+    if (ok && P.nfac == 1)
+      for (int e = P.fac[0].lin_beg; ok && e < P.fac[0].lin_end; ++e) ok = radial(P.lin[e]);
+    if (ok) {
+      for (int e = P.dyn[0].lhs_beg; e < P.dyn[0].lhs_end; ++e) P.rad_L[P.lin[e].m] -= P.lin[e].coef;
+      if (P.ngrp == 1) P.rad_O[P.grp[0].outer.m] += P.grp[0].outer.coef;
+      if (P.nfac == 1)
+        for (int e = P.fac[0].lin_beg; e < P.fac[0].lin_end; ++e) P.rad_F[P.lin[e].m] += P.lin[e].coef;
+      P.rad_nhp = P.dyn[0].noisy ? P.dyn[0].noise_qpow / 2 : 0;
+    }
+    P.rad_ok = ok ? 1 : 0;
+  }
   return PSS_OK;
 }
 
@@ -308,11 +332,6 @@ Geo make_geo(int64_t n) {
   g.nr = np;
   for (int q = 0; q < np; ++q) g.lg[q] = lg / np + (q < lg % np ? 1 : 0);
   return g;
-}
-
-int env_int(const char *name, int dflt) {
-  const char *v = std::getenv(name);
-  return (v && *v) ? std::atoi(v) : dflt;
 }
 
 const size_t SMEM_MAX = 227 * 1024;
@@ -385,6 +404,7 @@ int make_plan(pss_system *s) {
     }
     W = env_int("PSS_UPD_W", W);
     if (W < 1) W = 1;
+    while (W & (W - 1)) W &= W - 1; /* a power of two (the kernel indexes with shifts) */
     while (W > 1 && per * W > SMEM_MAX) W >>= 1;
     pl.upd_W = W;
     pl.upd_smem = per * W;
@@ -438,6 +458,7 @@ void carve_workspace(pss_system *s) {
   s->off_scratch = off; off += arr;
   s->off_ureal = off; off += align_up((size_t)s->N * s->rsize, 256);
   for (int j = 0; j < 3; ++j) { s->off_tw[j] = off; off += align_up((size_t)s->n[j] * s->csize, 256); }
+  s->off_rev = off; off += align_up((size_t)2 * (size_t)s->n[s->ndim - 1] * sizeof(unsigned short), 256);
   s->off_bar = off; off += 1024; /* v1: one 64-bit counter; v2: one 32-bit epoch flag per CTA */
   s->ws_need = off;
 }
@@ -454,7 +475,8 @@ template <typename T> const typename cplx_of<T>::type *twp(pss_system *s, int ax
 }
 
 template <typename T> int set_attrs(pss_system *s) {
-  CK(cudaFuncSetAttribute(k_update<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_MAX));
+  CK(cudaFuncSetAttribute(k_update<T, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_MAX));
+  CK(cudaFuncSetAttribute(k_update<T, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_MAX));
   CK(cudaFuncSetAttribute(k_rows<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_MAX));
   CK(cudaFuncSetAttribute(k_mid<-1, T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_MAX));
   CK(cudaFuncSetAttribute(k_mid<+1, T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_MAX));
@@ -509,6 +531,26 @@ template <typename T> int upload_twiddles(pss_system *s) {
     CK(cudaMemcpyAsync(s->ws + s->off_tw[j], tw.data(), tw.size() * sizeof(C), cudaMemcpyHostToDevice, s->stream));
     CK(cudaStreamSynchronize(s->stream)); /* tw is a stack-lifetime host buffer */
   }
+  /* digit-reversal tables of the last axis (k_update): slot_of[k], freq_of[s] */
+  {
+    const Geo &g = s->plan.geo[s->ndim - 1];
+    const int n = g.n;
+    std::vector<unsigned short> tab((size_t)2 * n);
+    int lgn = 0;
+    for (int q = 0; q < g.nr; ++q) lgn += g.lg[q];
+    for (int f = 0; f < n; ++f) {
+      int p = 0, rem = lgn, ff = f;
+      for (int q = 0; q < g.nr; ++q) {
+        rem -= g.lg[q];
+        p |= (ff & ((1 << g.lg[q]) - 1)) << rem;
+        ff >>= g.lg[q];
+      }
+      tab[(size_t)f] = (unsigned short)p;
+      tab[(size_t)n + p] = (unsigned short)f;
+    }
+    CK(cudaMemcpyAsync(s->ws + s->off_rev, tab.data(), tab.size() * sizeof(unsigned short), cudaMemcpyHostToDevice, s->stream));
+    CK(cudaStreamSynchronize(s->stream));
+  }
   return PSS_OK;
 }
 
@@ -553,15 +595,21 @@ template <typename T> int launch_update(pss_system *s, int prologue, uint64_t st
   a.psix = carr<T>(s, s->off_psix, 0);
   a.phat = carr<T>(s, s->off_phat, 0);
   a.tw = twp<T>(s, s->ndim - 1);
+  a.slot_of = reinterpret_cast<const unsigned short *>(s->ws + s->off_rev);
+  a.freq_of = a.slot_of + s->n[s->ndim - 1];
   a.M = arr_stride(s);
   a.n = (int)s->n[s->ndim - 1];
+  a.lgn = ilog2(a.n);
   a.nlines = (s->ndim == 3) ? (int)(P.nxh * s->n[1]) : P.nxh;
   a.W = s->plan.upd_W;
+  a.lgW = ilog2(a.W);
+  a.lg_ny = ilog2(s->n[1]);
   a.prologue = prologue;
   a.step = step;
   a.geo = s->plan.geo[s->ndim - 1];
   prof_mark(s, KIND_UPDATE, true);
-  k_update<T><<<s->plan.upd_blocks, s->plan.upd_threads, s->plan.upd_smem, s->stream>>>(P, a);
+  if (P.rad_ok) k_update<T, true><<<s->plan.upd_blocks, s->plan.upd_threads, s->plan.upd_smem, s->stream>>>(P, a);
+  else k_update<T, false><<<s->plan.upd_blocks, s->plan.upd_threads, s->plan.upd_smem, s->stream>>>(P, a);
   prof_mark(s, KIND_UPDATE, false);
   CKL("k_update");
   if (s->ndim == 3 && P.nfac > 0) return launch_mid<T>(s, +1, s->off_psix, P.nfac, s->plan.kx_keep_max, true);

@@ -183,7 +183,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_fused2d_v2(const __grid_constant
   if (noisew) {
     /* ============ noise warps: z(step s+1) is drawn while the transform warps work on step s ============ */
     if (!noisy || A.nsteps <= 0) return;
-    f2d::NoiseKey K;
+    NoiseKey K;
     K.k0 = P.seed_lo;
     K.k1 = P.seed_hi;
 #pragma unroll 1

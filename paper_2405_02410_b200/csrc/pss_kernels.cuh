@@ -24,94 +24,162 @@ template <typename T> struct UpdArgs {
   typename cplx_of<T>::type *psix;  /* [nfac][M] */
   typename cplx_of<T>::type *phat;  /* [ngrp][M] */
   const typename cplx_of<T>::type *tw;
+  const unsigned short *slot_of; /* slot_of[k]: shared-memory slot of frequency k after fft_dif (digit reversal) */
+  const unsigned short *freq_of; /* freq_of[s]: frequency held by slot s                                        */
   long long M;
-  int n;      /* last-axis length */
-  int nlines; /* nxh (2D) or nxh*ny (3D) */
-  int W;      /* lines per block */
+  int n, lgn;   /* last-axis length (a power of two) */
+  int nlines;   /* nxh (2D) or nxh*ny (3D) */
+  int W, lgW;   /* lines per block (a power of two) */
+  int lg_ny;    /* 3D: log2 ny */
   int prologue;
   unsigned long long step;
   Geo geo;
 };
 
+/* wavevector pieces shared by all modes of one last-axis line */
+template <typename T> struct LineQ {
+  T q0, q1, q2line;
+  int k0, k1, nyq;
+};
+template <typename T> __device__ __forceinline__ LineQ<T> make_line(const Program &P, int line, int lg_ny) {
+  LineQ<T> l;
+  if (P.ndim == 3) { l.k0 = line >> lg_ny; l.k1 = line & ((1 << lg_ny) - 1); } else { l.k0 = line; l.k1 = 0; }
+  l.q0 = (T)P.qs[0] * (T)signed_index(l.k0, P.n[0]);
+  l.nyq = (P.n[0] > 1 && 2 * l.k0 == P.n[0]) ? 1 : 0;
+  l.q2line = l.q0 * l.q0;
+  l.q1 = (T)0;
+  if (P.ndim == 3) {
+    l.q1 = (T)P.qs[1] * (T)signed_index(l.k1, P.n[1]);
+    if (P.n[1] > 1 && 2 * l.k1 == P.n[1]) l.nyq |= 2;
+    l.q2line += l.q1 * l.q1;
+  }
+  return l;
+}
+/* the mode (line, k) with k along the last axis; same arithmetic order as make_mode */
+template <typename T> __device__ __forceinline__ ModeQ<T> line_mode(const Program &P, const LineQ<T> &l, int k, int n, T qs_last) {
+  ModeQ<T> mq;
+  const T ql = qs_last * (T)signed_index(k, n);
+  const int last_nyq = (2 * k == n) ? 1 : 0;
+  mq.q[0] = l.q0;
+  if (P.ndim == 3) { mq.q[1] = l.q1; mq.q[2] = ql; mq.nyq = l.nyq | (last_nyq << 2); }
+  else { mq.q[1] = ql; mq.q[2] = (T)0; mq.nyq = l.nyq | (last_nyq << 1); }
+  mq.q2 = l.q2line + ql * ql;
+  return mq;
+}
+template <typename T> __device__ __forceinline__ T horner4(const T (&c)[5], T x) {
+  return c[0] + x * (c[1] + x * (c[2] + x * (c[3] + x * c[4])));
+}
+
 /* ------------------------------------------------------------------------------------------ */
-template <typename T>
-__global__ void __launch_bounds__(256) k_update(const __grid_constant__ Program P, const UpdArgs<T> A) {
+/* RAD: the "radial" fast path of pss_program.h (every per-mode coefficient is a polynomial in q^2) */
+template <typename T, bool RAD>
+__global__ void __launch_bounds__(256, sizeof(T) == 4 ? 3 : 2) k_update(const __grid_constant__ Program P, const UpdArgs<T> A) {
   typedef typename cplx_of<T>::type C;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   C *sm = reinterpret_cast<C *>(smem_raw);
-  const int n = A.n, W = A.W;
+  const int n = A.n, W = A.W, lgn = A.lgn, lgW = A.lgW;
   const int line0 = blockIdx.x * W;
   const int nl = min(W, A.nlines - line0);
   const int nb0 = max(P.ngrp, P.ndyn);
   const int RS = (nb0 + (P.nfac > 1 ? 1 : 0)) * W; /* columns per smem row */
   const int tid = threadIdx.x, nt = blockDim.x;
-  const int ny3 = (P.ndim == 3) ? P.n[1] : 1;
+  const T qs_last = (T)P.qs[P.ndim - 1];
+  const T dt = (T)P.dt, invN = (T)P.invN;
+  const C zero = mk<C, T>((T)0, (T)0);
+  T radL[5], radO[5], radF[5];
+#pragma unroll
+  for (int i = 0; i < 5; ++i) { radL[i] = (T)P.rad_L[i]; radO[i] = (T)P.rad_O[i]; radF[i] = (T)P.rad_F[i]; }
 
   /* ---- phase A: forward FFT of the groups along the last axis ---- */
-  if (!A.prologue) {
-    if (P.ngrp > 0) {
-      for (int g = 0; g < P.ngrp; ++g) {
-        const C *src = A.phat + (size_t)g * A.M + (size_t)line0 * n;
-        for (int idx = tid; idx < n * W; idx += nt) {
-          const int c = idx / n, j = idx - c * n;
-          sm[(size_t)j * RS + g * W + c] = (c < nl) ? src[(size_t)c * n + j] : mk<C, T>((T)0, (T)0);
-        }
+  if (!A.prologue && P.ngrp > 0) {
+    for (int g = 0; g < P.ngrp; ++g) {
+      const C *src = A.phat + (size_t)g * A.M + (size_t)line0 * n;
+      for (int idx = tid; idx < (W << lgn); idx += nt) {
+        const int c = idx >> lgn, j = idx & (n - 1);
+        sm[(size_t)j * RS + g * W + c] = (c < nl) ? src[idx] : zero;
       }
-      __syncthreads();
-      fft_dif<-1, T>(A.geo, sm, A.tw, P.ngrp * W, RS);
     }
+    __syncthreads();
+    fft_dif<-1, T>(A.geo, sm, A.tw, P.ngrp * W, RS);
   }
   /* ---- phase B: Eq. 15 + Eq. 16 + Eq. 18 per mode, natural order over k (coalesced state access) ---- */
-  for (int idx = tid; idx < n * W; idx += nt) {
-    const int c = idx / n, k = idx - c * n;
-    if (c >= nl) continue;
+  for (int c = 0; c < nl; ++c) {
     const int line = line0 + c;
-    const int slot = geo_slot(A.geo, k);
-    C *srow = sm + (size_t)slot * RS + c;
-    C phi[PSS_P_MAX_DYN];
-#pragma unroll
-    for (int i = 0; i < PSS_P_MAX_DYN; ++i)
-      phi[i] = (i < P.ndyn) ? A.state[(size_t)i * A.M + (size_t)line * n + k] : mk<C, T>((T)0, (T)0);
-    if (!A.prologue) {
-      int k0, k1, k2;
-      if (P.ndim == 3) { k0 = line / ny3; k1 = line - k0 * ny3; k2 = k; } else { k0 = line; k1 = k; k2 = 0; }
-      const ModeQ<T> mq = make_mode<T>(P, k0, k1, k2);
-      C out[PSS_P_MAX_DYN];
-#pragma unroll
-      for (int i = 0; i < PSS_P_MAX_DYN; ++i) {
-        if (i < P.ndyn) {
-          const DDyn &d = P.dyn[i];
-          C N = mk<C, T>((T)0, (T)0);
-          for (int g = 0; g < P.ngrp; ++g)
-            if (P.grp[g].target == i) N = cadd(N, cmul(eval_op<T>(P.grp[g].outer, mq), srow[g * W]));
-          for (int e = d.lin_beg; e < d.lin_end; ++e) N = cadd(N, cmul(eval_op<T>(P.lin[e], mq), sel4(phi, P.lin[e].src)));
-          C L = mk<C, T>((T)0, (T)0);
-          for (int e = d.lhs_beg; e < d.lhs_end; ++e) L = csub(L, eval_op<T>(P.lin[e], mq));
-          C num = mk<C, T>(phi[i].x + (T)P.dt * N.x, phi[i].y + (T)P.dt * N.y);
+    const LineQ<T> lq = make_line<T>(P, line, A.lg_ny);
+    for (int k = tid; k < n; k += nt) {
+      C *srow = sm + (size_t)A.slot_of[k] * RS + c;
+      const size_t gi = (size_t)line * n + k;
+      if (RAD) {
+        const C phi = A.state[gi];
+        if (!A.prologue) {
+          const ModeQ<T> mq = line_mode<T>(P, lq, k, n, qs_last);
+          C num = phi;
+          if (P.ngrp > 0) {
+            const T o = dt * horner4<T>(radO, mq.q2);
+            const C pq = srow[0];
+            num.x += o * pq.x;
+            num.y += o * pq.y;
+          }
+          const DDyn &d = P.dyn[0];
           if (d.noisy) {
-            const T amp = noise_amp<T>(d, mq);
-            const C z = noise_z<T>(P, d.field_id, A.step, k0, k1, k2);
+            T qa = (T)d.noise_c;
+            for (int i = 0; i < P.rad_nhp; ++i) qa *= mq.q2;
+            const T amp = sqrt(qa);
+            const C z = noise_z<T>(P, d.field_id, A.step, lq.k0, P.ndim == 3 ? lq.k1 : k, P.ndim == 3 ? k : 0);
             num.x += amp * z.x;
             num.y += amp * z.y;
           }
-          const C den = mk<C, T>((T)1 - (T)P.dt * L.x, -(T)P.dt * L.y);
-          const T id = (T)1 / (den.x * den.x + den.y * den.y);
-          const C q = cmulc(num, den);
-          out[i] = mk<C, T>(q.x * id, q.y * id);
+          const T inv = (T)1 / ((T)1 - dt * horner4<T>(radL, mq.q2));
+          const C out = mk<C, T>(num.x * inv, num.y * inv);
+          A.state[gi] = out;
+          srow[0] = out;
         } else {
-          out[i] = mk<C, T>((T)0, (T)0);
+          srow[0] = phi;
         }
+        continue;
       }
+      C phi[PSS_P_MAX_DYN];
 #pragma unroll
-      for (int i = 0; i < PSS_P_MAX_DYN; ++i)
-        if (i < P.ndyn) {
-          A.state[(size_t)i * A.M + (size_t)line * n + k] = out[i];
-          srow[i * W] = out[i];
+      for (int i = 0; i < PSS_P_MAX_DYN; ++i) phi[i] = (i < P.ndyn) ? A.state[(size_t)i * A.M + gi] : zero;
+      if (!A.prologue) {
+        const ModeQ<T> mq = line_mode<T>(P, lq, k, n, qs_last);
+        C out[PSS_P_MAX_DYN];
+#pragma unroll
+        for (int i = 0; i < PSS_P_MAX_DYN; ++i) {
+          if (i < P.ndyn) {
+            const DDyn &d = P.dyn[i];
+            C N = zero;
+            for (int g = 0; g < P.ngrp; ++g)
+              if (P.grp[g].target == i) N = cadd(N, cmul(eval_op<T>(P.grp[g].outer, mq), srow[g * W]));
+            for (int e = d.lin_beg; e < d.lin_end; ++e) N = cadd(N, cmul(eval_op<T>(P.lin[e], mq), sel4(phi, P.lin[e].src)));
+            C L = zero;
+            for (int e = d.lhs_beg; e < d.lhs_end; ++e) L = csub(L, eval_op<T>(P.lin[e], mq));
+            C num = mk<C, T>(phi[i].x + dt * N.x, phi[i].y + dt * N.y);
+            if (d.noisy) {
+              const T amp = noise_amp<T>(d, mq);
+              const C z = noise_z<T>(P, d.field_id, A.step, lq.k0, P.ndim == 3 ? lq.k1 : k, P.ndim == 3 ? k : 0);
+              num.x += amp * z.x;
+              num.y += amp * z.y;
+            }
+            const C den = mk<C, T>((T)1 - dt * L.x, -dt * L.y);
+            const T id = (T)1 / (den.x * den.x + den.y * den.y);
+            const C q = cmulc(num, den);
+            out[i] = mk<C, T>(q.x * id, q.y * id);
+          } else {
+            out[i] = zero;
+          }
         }
-    } else {
 #pragma unroll
-      for (int i = 0; i < PSS_P_MAX_DYN; ++i)
-        if (i < P.ndyn) srow[i * W] = phi[i];
+        for (int i = 0; i < PSS_P_MAX_DYN; ++i)
+          if (i < P.ndyn) {
+            A.state[(size_t)i * A.M + gi] = out[i];
+            srow[i * W] = out[i];
+          }
+      } else {
+#pragma unroll
+        for (int i = 0; i < PSS_P_MAX_DYN; ++i)
+          if (i < P.ndyn) srow[i * W] = phi[i];
+      }
     }
   }
   __syncthreads();
@@ -125,7 +193,7 @@ __global__ void __launch_bounds__(256) k_update(const __grid_constant__ Program 
       const int line = line0 + c;
       bool kp;
       if (P.ndim == 3) {
-        const int k0 = line / ny3, k1 = line - k0 * ny3;
+        const int k0 = line >> A.lg_ny, k1 = line & ((1 << A.lg_ny) - 1);
         kp = keep_axis(P.dealias, F.order, k0, P.n[0]) && keep_axis(P.dealias, F.order, k1, P.n[1]);
       } else {
         kp = keep_axis(P.dealias, F.order, line, P.n[0]);
@@ -133,23 +201,27 @@ __global__ void __launch_bounds__(256) k_update(const __grid_constant__ Program 
       if (kp) keepmask |= 1u << c;
     }
     if (keepmask == 0) continue; /* the whole tile is masked: psix stays zero (zeroed at bind) */
-    for (int idx = tid; idx < n * W; idx += nt) {
-      const int c = idx % W, s = idx / W;
+    for (int idx = tid; idx < (n << lgW); idx += nt) {
+      const int c = idx & (W - 1), s = idx >> lgW;
       C *srow = sm + (size_t)s * RS + c;
-      C v = mk<C, T>((T)0, (T)0);
+      C v = zero;
       if ((keepmask >> c) & 1u) {
-        const int k = geo_rev(A.geo, s);
+        const int k = A.freq_of[s];
         if (keep_axis(P.dealias, F.order, k, n)) {
-          const int line = line0 + c;
-          int k0, k1, k2;
-          if (P.ndim == 3) { k0 = line / ny3; k1 = line - k0 * ny3; k2 = k; } else { k0 = line; k1 = k; k2 = 0; }
-          const ModeQ<T> mq = make_mode<T>(P, k0, k1, k2);
-          C phi[PSS_P_MAX_DYN];
+          const LineQ<T> lq = make_line<T>(P, line0 + c, A.lg_ny);
+          const ModeQ<T> mq = line_mode<T>(P, lq, k, n, qs_last);
+          if (RAD) {
+            const T fc = horner4<T>(radF, mq.q2) * invN;
+            const C ph = srow[0];
+            v = mk<C, T>(ph.x * fc, ph.y * fc);
+          } else {
+            C phi[PSS_P_MAX_DYN];
 #pragma unroll
-          for (int i = 0; i < PSS_P_MAX_DYN; ++i) phi[i] = (i < P.ndyn) ? srow[i * W] : mk<C, T>((T)0, (T)0);
-          for (int e = F.lin_beg; e < F.lin_end; ++e) v = cadd(v, cmul(eval_op<T>(P.lin[e], mq), sel4(phi, P.lin[e].src)));
-          v.x *= (T)P.invN;
-          v.y *= (T)P.invN;
+            for (int i = 0; i < PSS_P_MAX_DYN; ++i) phi[i] = (i < P.ndyn) ? srow[i * W] : zero;
+            for (int e = F.lin_beg; e < F.lin_end; ++e) v = cadd(v, cmul(eval_op<T>(P.lin[e], mq), sel4(phi, P.lin[e].src)));
+            v.x *= invN;
+            v.y *= invN;
+          }
         }
       }
       srow[wb * W] = v;
@@ -157,9 +229,9 @@ __global__ void __launch_bounds__(256) k_update(const __grid_constant__ Program 
     __syncthreads();
     fft_dit<+1, T>(A.geo, sm + wb * W, A.tw, W, RS);
     C *dst = A.psix + (size_t)f * A.M + (size_t)line0 * n;
-    for (int idx = tid; idx < n * W; idx += nt) {
-      const int c = idx / n, j = idx - c * n;
-      if ((keepmask >> c) & 1u) dst[(size_t)c * n + j] = sm[(size_t)j * RS + wb * W + c];
+    for (int idx = tid; idx < (W << lgn); idx += nt) {
+      const int c = idx >> lgn, j = idx & (n - 1);
+      if ((keepmask >> c) & 1u) dst[idx] = sm[(size_t)j * RS + wb * W + c];
     }
     __syncthreads();
   }

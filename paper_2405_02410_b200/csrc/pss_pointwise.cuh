@@ -40,15 +40,19 @@ template <typename T> __device__ __forceinline__ typename cplx_of<T>::type eval_
   typedef typename cplx_of<T>::type C;
   if ((op.zflags & 7 & mq.nyq) || ((op.zflags & 8) && mq.q2 == (T)0)) return mk<C, T>((T)0, (T)0);
   T r = (T)op.coef;
-  for (int i = 0; i < op.m; ++i) r *= mq.q2;
+  {
+    T bq = mq.q2;
+    for (int m = op.m; m > 0; m >>= 1) { if (m & 1) r *= bq; bq *= bq; }
+  }
   if (op.p > 0) {
-    const T inv = (T)1 / sqrt(mq.q2);
-    for (int i = 0; i < op.p; ++i) r *= inv;
+    T bq = (T)1 / sqrt(mq.q2);
+    for (int m = op.p; m > 0; m >>= 1) { if (m & 1) r *= bq; bq *= bq; }
   }
   int s = 0;
 #pragma unroll
   for (int j = 0; j < 3; ++j) {
-    for (int i = 0; i < op.a[j]; ++i) r *= mq.q[j];
+    T bq = mq.q[j];
+    for (int m = op.a[j]; m > 0; m >>= 1) { if (m & 1) r *= bq; bq *= bq; }
     s += op.a[j];
   }
   switch (s & 3) {
@@ -111,6 +115,73 @@ __device__ __forceinline__ void gauss_pair(const uint32_t w[4], double &g1, doub
   g2 = r * s;
 }
 
+/* ---- noise (Eq. 16): Philox4x32-10 + Box-Muller, lean fp32 path: only the two words the
+ * fp32 uniforms use (same counter, same words, same uniforms as noise_block/gauss_pair), the step-invariant half of
+ * round 1 left to the compiler to hoist, and own fp32 ln / sin / cos kernels
+ * (coefficients fitted for this file; each within ~1 ulp of the exact value over all 2^24 inputs). ---- */
+struct NoiseKey {
+  uint32_t c2, c3;   /* counter words 2, 3: step_lo, ((step_hi & 0xffff) << 16) | field */
+  uint32_t k0, k1;   /* key = seed */
+};
+
+__device__ __forceinline__ void philox_w01(uint32_t c0, uint32_t c1, const NoiseKey &K, uint32_t &w0, uint32_t &w1) {
+  uint32_t c2 = K.c2, c3 = K.c3, k0 = K.k0, k1 = K.k1;
+#pragma unroll
+  for (int r = 0; r < 10; ++r) {
+    const uint32_t hi0 = __umulhi(0xD2511F53u, c0), lo0 = 0xD2511F53u * c0;
+    const uint32_t hi1 = __umulhi(0xCD9E8D57u, c2), lo1 = 0xCD9E8D57u * c2;
+    const uint32_t n0 = hi1 ^ c1 ^ k0, n2 = hi0 ^ c3 ^ k1;
+    c0 = n0; c1 = lo1; c2 = n2; c3 = lo0;
+    k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
+  }
+  w0 = c0; w1 = c1;
+}
+
+/* sqrt(-ln u1) * (cos 2 pi u2, sin 2 pi u2) with u1 = ((w0>>8)+1) 2^-24 in (0,1], u2 = (w1>>8) 2^-24 in [0,1):
+ * this is (g1 + i g2)/sqrt(2) of the Box-Muller pair g = sqrt(-2 ln u1) (cos, sin). */
+__device__ __forceinline__ float2 box_muller_half(uint32_t w0, uint32_t w1) {
+  /* ln u1: u1 = m 2^e, m in [2/3, 4/3); ln m = f - f^2/2 + f^3 P(f), f = m - 1 */
+  const float u1 = (float)((w0 >> 8) + 1u) * (1.0f / 16777216.0f);
+  const int iu = __float_as_int(u1);
+  const int e = (iu - 0x3f2aaaab) & 0xff800000;
+  const float f = __int_as_float(iu - e) - 1.0f;
+  const float fe = (float)e * 1.1920928955078125e-07f;
+  float p = -0.12429866194725037f;
+  p = fmaf(p, f, 0.13433773815631866f);
+  p = fmaf(p, f, -0.12287236750125885f);
+  p = fmaf(p, f, 0.14116978645324707f);
+  p = fmaf(p, f, -0.166733980178833f);
+  p = fmaf(p, f, 0.2000383585691452f);
+  p = fmaf(p, f, -0.24999943375587463f);
+  p = fmaf(p, f, 0.33333319425582886f);
+  const float f2 = f * f;
+  const float lnm = fmaf(p * f, f2, -0.5f * f2) + f;
+  const float x = -fmaf(fe, 0.693147182464599609375f, lnm);          /* -ln u1 >= 0 */
+  /* sqrt by rsqrt + one Newton step; x = 0 (u1 = 1) gives 0 */
+  const float y = rsqrtf(fmaxf(x, 1e-30f));
+  float r = x * y;
+  r = fmaf(0.5f * y, fmaf(-r, r, x), r);
+  /* angle 2 pi j / 2^24: nearest quadrant q, remainder phi in [-pi/4, pi/4) exactly representable */
+  const uint32_t j = w1 >> 8;
+  const uint32_t qq = (j + (1u << 21)) >> 22;
+  const int rem = (int)j - (int)(qq << 22);
+  const float phi = (float)rem * 3.7450702829191576e-07f;             /* 2 pi / 2^24 */
+  const float u = phi * phi;
+  float sp = 2.7249941467744065e-06f, cp = -4.133496076974552e-06f;
+  sp = fmaf(sp, u, -0.00019840087043121457f);
+  cp = fmaf(cp, u, 2.896795376727823e-05f);
+  sp = fmaf(sp, u, 0.008333331905305386f);
+  cp = fmaf(cp, u, -0.0013901740312576294f);
+  sp = fmaf(sp, u, -0.1666666716337204f);
+  cp = fmaf(cp, u, 0.04166676476597786f);
+  const float sn = fmaf(phi * u, sp, phi);
+  const float cn = fmaf(u * u, cp, fmaf(-0.5f, u, 1.0f));
+  const float ca = (qq & 1u) ? sn : cn, sa = (qq & 1u) ? cn : sn;     /* |cos|, |sin| carriers */
+  const float c = ((qq + 1u) & 2u) ? -ca : ca;                        /* q = 1, 2 -> negative cosine */
+  const float sgn = (qq & 2u) ? -sa : sa;                             /* q = 2, 3 -> negative sine   */
+  return make_float2(r * c, r * sgn);
+}
+
 /* unit-variance Hermitian complex Gaussian at logical mode (k0,k1,k2)  (Eq. 16, 134) */
 template <typename T>
 __device__ __forceinline__ typename cplx_of<T>::type noise_z(const Program &P, int field, unsigned long long step,
@@ -134,6 +205,33 @@ __device__ __forceinline__ typename cplx_of<T>::type noise_z(const Program &P, i
   if (mp == m) return mk<C, T>(g1, (T)0);
   const T h = (T)0.70710678118654752440;
   return mk<C, T>(g1 * h, (m < mp) ? g2 * h : -(g2 * h));
+}
+
+/* fp32: the same stream through the lean path (two words, own ln/sin/cos) */
+template <>
+__device__ __forceinline__ float2 noise_z<float>(const Program &P, int field, unsigned long long step, int k0, int k1, int k2) {
+  const long long n1 = P.n[1], n2 = P.n[2], nxh = P.nxh;
+  long long m = ((long long)k2 * n1 + k1) * nxh + k0;
+  NoiseKey K;
+  K.k0 = P.seed_lo;
+  K.k1 = P.seed_hi;
+  K.c2 = (uint32_t)(step & 0xffffffffu);
+  K.c3 = (uint32_t)((((step >> 32) & 0xffffu) << 16) | ((uint32_t)field & 0xffffu));
+  const bool on_plane = (k0 == 0) || (2 * k0 == P.n[0]);
+  bool self = false, other = false;
+  if (on_plane) {
+    const long long p1 = (k1 == 0) ? 0 : n1 - k1, p2 = (k2 == 0) ? 0 : n2 - k2;
+    const long long mp = (p2 * n1 + p1) * nxh + k0;
+    self = (mp == m);
+    other = (mp < m);
+    m = other ? mp : m;
+  }
+  uint32_t w0, w1;
+  philox_w01((uint32_t)((unsigned long long)m & 0xffffffffu), (uint32_t)((unsigned long long)m >> 32), K, w0, w1);
+  float2 z = box_muller_half(w0, w1);
+  if (self) z = make_float2(z.x * 1.41421356237309504880f, 0.f);
+  else if (other) z.y = -z.y;
+  return z;
 }
 
 /* sqrt(2 D |q|^a dt N / dV)  (A1) */

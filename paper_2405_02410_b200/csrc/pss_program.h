@@ -79,6 +79,13 @@ struct Program {
   DGroup grp[PSS_P_MAX_GRP];
   DTerm term[PSS_P_MAX_TERM];
   DOp lin[PSS_P_MAX_LIN];
+  /* "radial" fast path (set by the host when it applies): one dynamic field, at most one product group and one
+   * factor, no explicit linear terms, every monomial a pure power (q^2)^m with m <= 4, noise power even and >= 0.
+   * Then every per-mode coefficient is a polynomial in q^2 (Horner, ascending coefficients):
+   *   L(q) = rad_L(q^2), outer(q) = rad_O(q^2), factor(q) = rad_F(q^2), noise amp = sqrt(noise_c (q^2)^rad_nhp). */
+  int32_t rad_ok;
+  int32_t rad_nhp;
+  double rad_L[5], rad_O[5], rad_F[5];
 };
 
 /* radix schedule of one in-shared-memory FFT of length n = prod R[i] */
