@@ -323,6 +323,8 @@ int build_program(pss_system *s) {
 }
 
 /* ---- launch plan ----------------------------------------------------------------------- */
+int geo_pad_h(const Geo &g, int p) { return p + (p >> g.sh[0]) + (p >> g.sh[1]) + (p >> g.sh[2]); }
+
 Geo make_geo(int64_t n) {
   Geo g;
   std::memset(&g, 0, sizeof(g));
@@ -331,6 +333,11 @@ Geo make_geo(int64_t n) {
   const int np = (lg + 3) / 4;
   g.nr = np;
   for (int q = 0; q < np; ++q) g.lg[q] = lg / np + (q < lg % np ? 1 : 0);
+  /* pad rows at the digit boundaries of the slot index (the last pass's digit sits in the low bits) */
+  int b = 0, k = 0;
+  for (int i = 0; i < 3; ++i) g.sh[i] = 31;
+  for (int q = np - 1; q >= 1; --q) { b += g.lg[q]; g.sh[k++] = b; }
+  g.npad = geo_pad_h(g, (int)n - 1) + 1;
   return g;
 }
 
@@ -382,7 +389,7 @@ int make_plan(pss_system *s) {
   }
   if (s->ndim == 1) {
     const size_t bufs = (size_t)(P.nfac + P.ngrp);
-    pl.one_smem = bufs * (size_t)s->n[0] * cs;
+    pl.one_smem = bufs * (size_t)pl.geo[0].npad * cs;
     if (pl.one_smem > SMEM_MAX) return PSS_EUNSUPPORTED;
     if (pl.one_smem < 16) pl.one_smem = 16;
     pl.one_threads = round_threads(s->n[0] / 4);
@@ -393,7 +400,7 @@ int make_plan(pss_system *s) {
     const int64_t n = s->n[s->ndim - 1];
     const int64_t nlines = (s->ndim == 3) ? (int64_t)nxh * s->n[1] : nxh;
     const int nb0 = P.ngrp > P.ndyn ? P.ngrp : P.ndyn;
-    const size_t per = (size_t)(nb0 + (P.nfac > 1 ? 1 : 0)) * (size_t)n * cs;
+    const size_t per = (size_t)(nb0 + (P.nfac > 1 ? 1 : 0)) * (size_t)pl.geo[s->ndim - 1].npad * cs;
     if (per > SMEM_MAX) return PSS_EUNSUPPORTED;
     int W = 1;
     for (int cand = 8; cand >= 1; cand >>= 1) {
@@ -415,7 +422,7 @@ int make_plan(pss_system *s) {
   if (P.ngrp > 0) {
     const int64_t nx = s->n[0];
     const int64_t R = s->N / nx;
-    const size_t per = (size_t)(P.nfac + (P.ngrp > 1 ? 1 : 0)) * (size_t)nx * cs;
+    const size_t per = (size_t)(P.nfac + (P.ngrp > 1 ? 1 : 0)) * (size_t)pl.geo[0].npad * cs;
     if (per > SMEM_MAX) return PSS_EUNSUPPORTED;
     const int wc_sector = (cs == 8) ? 2 : 1; /* 2*Wc complex = one 32-byte sector */
     int Wc = 1;
@@ -437,10 +444,10 @@ int make_plan(pss_system *s) {
   if (s->ndim == 3) {
     int W = (int)(128 / cs);
     if (W > s->n[2]) W = (int)s->n[2];
-    while ((size_t)W * s->n[1] * cs > SMEM_MAX && W > 1) W >>= 1;
-    if ((size_t)W * s->n[1] * cs > SMEM_MAX) return PSS_EUNSUPPORTED;
+    while ((size_t)W * pl.geo[1].npad * cs > SMEM_MAX && W > 1) W >>= 1;
+    if ((size_t)W * pl.geo[1].npad * cs > SMEM_MAX) return PSS_EUNSUPPORTED;
     pl.mid_W = W;
-    pl.mid_smem = (size_t)W * s->n[1] * cs;
+    pl.mid_smem = (size_t)W * pl.geo[1].npad * cs;
     pl.mid_threads = round_threads((s->n[1] / 8) * W);
   }
   return PSS_OK;
@@ -545,7 +552,7 @@ template <typename T> int upload_twiddles(pss_system *s) {
         p |= (ff & ((1 << g.lg[q]) - 1)) << rem;
         ff >>= g.lg[q];
       }
-      tab[(size_t)f] = (unsigned short)p;
+      tab[(size_t)f] = (unsigned short)geo_pad_h(g, p);
       tab[(size_t)n + p] = (unsigned short)f;
     }
     CK(cudaMemcpyAsync(s->ws + s->off_rev, tab.data(), tab.size() * sizeof(unsigned short), cudaMemcpyHostToDevice, s->stream));
@@ -713,7 +720,7 @@ template <typename T> int do_set_field(pss_system *s, int slot, const void *src,
   a.geo = s->plan.geo[0];
   const int64_t R = s->N / s->n[0];
   const unsigned blocks = (unsigned)(a.single ? R : R / 2);
-  k_user_x<-1, T><<<blocks, round_threads(s->n[0] / 4), (size_t)s->n[0] * sizeof(typename cplx_of<T>::type), s->stream>>>(a);
+  k_user_x<-1, T><<<blocks, round_threads(s->n[0] / 4), (size_t)s->plan.geo[0].npad * sizeof(typename cplx_of<T>::type), s->stream>>>(a);
   CKL("k_user_x");
   if (s->ndim == 3) {
     const int rc = launch_mid<T>(s, -1, s->off_state + (size_t)slot * (size_t)arr_stride(s) * s->csize, 1, s->P.nxh);
@@ -726,7 +733,7 @@ template <typename T> int do_set_field(pss_system *s, int slot, const void *src,
     l.n = (int)s->n[s->ndim - 1];
     l.nlines = (int)(s->M / l.n);
     l.geo = s->plan.geo[s->ndim - 1];
-    k_last<-1, T><<<l.nlines, round_threads(l.n / 4), (size_t)l.n * sizeof(typename cplx_of<T>::type), s->stream>>>(l);
+    k_last<-1, T><<<l.nlines, round_threads(l.n / 4), (size_t)l.geo.npad * sizeof(typename cplx_of<T>::type), s->stream>>>(l);
     CKL("k_last");
   }
   s->psix_valid = false;
@@ -745,7 +752,7 @@ template <typename T> int do_get_field(pss_system *s, int slot, void *dst, int o
     l.n = (int)s->n[s->ndim - 1];
     l.nlines = (int)(s->M / l.n);
     l.geo = s->plan.geo[s->ndim - 1];
-    k_last<+1, T><<<l.nlines, round_threads(l.n / 4), (size_t)l.n * sizeof(C), s->stream>>>(l);
+    k_last<+1, T><<<l.nlines, round_threads(l.n / 4), (size_t)l.geo.npad * sizeof(C), s->stream>>>(l);
     CKL("k_last");
   }
   if (s->ndim == 3) {
@@ -764,7 +771,7 @@ template <typename T> int do_get_field(pss_system *s, int slot, void *dst, int o
   a.geo = s->plan.geo[0];
   const int64_t R = s->N / s->n[0];
   const unsigned blocks = (unsigned)(a.single ? R : R / 2);
-  k_user_x<+1, T><<<blocks, round_threads(s->n[0] / 4), (size_t)s->n[0] * sizeof(C), s->stream>>>(a);
+  k_user_x<+1, T><<<blocks, round_threads(s->n[0] / 4), (size_t)s->plan.geo[0].npad * sizeof(C), s->stream>>>(a);
   CKL("k_user_x");
   if (!on_device) {
     CK(cudaMemcpyAsync(dst, s->ws + s->off_ureal, (size_t)s->N * sizeof(T), cudaMemcpyDeviceToHost, s->stream));

@@ -2,7 +2,7 @@
  * pss_fft.cuh — in-shared-memory FFT building blocks (sm_100a).
  *
  * A line of n = prod R_i complex points lives in shared memory, W lines interleaved:
- * element (j, c) at buf[j*W + c].  Transforms are done IN PLACE without any reordering pass:
+ * element (j, c) at buf[geo_pad(j)*W + c] (rows padded against bank conflicts, see Geo).  Transforms are done IN PLACE without any reordering pass:
  *   fft_dif : natural order in  -> digit-reversed order out   (decimation in frequency)
  *   fft_dit : digit-reversed in -> natural order out           (its exact transpose)
  * The callers pair them so the digit-reversed order only ever meets pointwise work, which does
@@ -111,24 +111,34 @@ __device__ __forceinline__ int geo_slot(const Geo &g, int f) { /* index -> slot 
   return p;
 }
 
+/* padded shared-memory row of slot p (see Geo) */
+__device__ __forceinline__ int geo_pad(const Geo &g, int p) { return p + (p >> g.sh[0]) + (p >> g.sh[1]) + (p >> g.sh[2]); }
+/* padded row stride of the digit whose field starts at slot bit lo (lo is 0 or one of g.sh) */
+__device__ __forceinline__ int geo_stride(const Geo &g, int lo) {
+  int w = 1 << lo;
+#pragma unroll
+  for (int i = 0; i < 3; ++i) if (g.sh[i] <= lo) w += 1 << (lo - g.sh[i]);
+  return w;
+}
+
 /* one radix-2^LGR pass over `ncol` interleaved columns: element (j, c) at buf[j*rs + c], c < ncol <= rs
  * (several buffers of W columns each sit side by side in one row of rs columns).  lgL = log2 of the current sub-length L, lgn = log2 n.
  * DIT = false: butterfly then twiddle (DIF).  DIT = true: twiddle then butterfly. */
 template <int LGR, int SGN, bool DIT, typename T>
-__device__ __forceinline__ void fft_pass(typename cplx_of<T>::type *buf, const typename cplx_of<T>::type *__restrict__ tw,
+__device__ __forceinline__ void fft_pass(const Geo &g, typename cplx_of<T>::type *buf, const typename cplx_of<T>::type *__restrict__ tw,
                                          int lgn, int lgL, int ncol, int rs) {
   typedef typename cplx_of<T>::type C;
   constexpr int R = 1 << LGR;
   const int lgLs = lgL - LGR;          /* log2 of the leg stride L/R */
   const int nb = (1 << (lgn - LGR));   /* butterflies per column     */
   const int total = nb * ncol;
+  const int ls = rs * geo_stride(g, lgLs); /* padded leg stride */
   for (int idx = threadIdx.x; idx < total; idx += blockDim.x) {
     const int c = idx % ncol;
     const int b = idx / ncol;
     const int i = b & ((1 << lgLs) - 1);
     const int blk = b >> lgLs;
-    C *p = buf + (size_t)((blk << lgL) + i) * rs + c;
-    const int ls = rs << lgLs;
+    C *p = buf + (size_t)geo_pad(g, (blk << lgL) + i) * rs + c;
     const int tws = i << (lgn - lgL);  /* twiddle index step: w_L^i = tw[i * n/L] */
     C v[R];
 #pragma unroll
@@ -154,13 +164,13 @@ __device__ __forceinline__ void fft_pass(typename cplx_of<T>::type *buf, const t
 }
 
 template <int SGN, bool DIT, typename T>
-__device__ __forceinline__ void fft_pass_any(int lgr, typename cplx_of<T>::type *buf,
+__device__ __forceinline__ void fft_pass_any(const Geo &g, int lgr, typename cplx_of<T>::type *buf,
                                              const typename cplx_of<T>::type *__restrict__ tw, int lgn, int lgL, int ncol, int rs) {
   switch (lgr) {
-    case 1: fft_pass<1, SGN, DIT, T>(buf, tw, lgn, lgL, ncol, rs); break;
-    case 2: fft_pass<2, SGN, DIT, T>(buf, tw, lgn, lgL, ncol, rs); break;
-    case 3: fft_pass<3, SGN, DIT, T>(buf, tw, lgn, lgL, ncol, rs); break;
-    default: fft_pass<4, SGN, DIT, T>(buf, tw, lgn, lgL, ncol, rs); break;
+    case 1: fft_pass<1, SGN, DIT, T>(g, buf, tw, lgn, lgL, ncol, rs); break;
+    case 2: fft_pass<2, SGN, DIT, T>(g, buf, tw, lgn, lgL, ncol, rs); break;
+    case 3: fft_pass<3, SGN, DIT, T>(g, buf, tw, lgn, lgL, ncol, rs); break;
+    default: fft_pass<4, SGN, DIT, T>(g, buf, tw, lgn, lgL, ncol, rs); break;
   }
 }
 
@@ -172,7 +182,7 @@ __device__ __forceinline__ void fft_dif(const Geo &g, typename cplx_of<T>::type 
   for (int q = 0; q < g.nr; ++q) lgn += g.lg[q];
   int lgL = lgn;
   for (int q = 0; q < g.nr; ++q) {
-    fft_pass_any<SGN, false, T>(g.lg[q], buf, tw, lgn, lgL, ncol, rs);
+    fft_pass_any<SGN, false, T>(g, g.lg[q], buf, tw, lgn, lgL, ncol, rs);
     lgL -= g.lg[q];
     __syncthreads();
   }
@@ -187,7 +197,7 @@ __device__ __forceinline__ void fft_dit(const Geo &g, typename cplx_of<T>::type 
   int lgL = 0;
   for (int q = g.nr - 1; q >= 0; --q) {
     lgL += g.lg[q];
-    fft_pass_any<SGN, true, T>(g.lg[q], buf, tw, lgn, lgL, ncol, rs);
+    fft_pass_any<SGN, true, T>(g, g.lg[q], buf, tw, lgn, lgL, ncol, rs);
     __syncthreads();
   }
 }

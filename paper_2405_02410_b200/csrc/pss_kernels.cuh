@@ -24,7 +24,7 @@ template <typename T> struct UpdArgs {
   typename cplx_of<T>::type *psix;  /* [nfac][M] */
   typename cplx_of<T>::type *phat;  /* [ngrp][M] */
   const typename cplx_of<T>::type *tw;
-  const unsigned short *slot_of; /* slot_of[k]: shared-memory slot of frequency k after fft_dif (digit reversal) */
+  const unsigned short *slot_of; /* slot_of[k]: PADDED shared-memory row of frequency k after fft_dif (digit reversal) */
   const unsigned short *freq_of; /* freq_of[s]: frequency held by slot s                                        */
   long long M;
   int n, lgn;   /* last-axis length (a power of two) */
@@ -96,7 +96,7 @@ __global__ void __launch_bounds__(256, sizeof(T) == 4 ? 3 : 2) k_update(const __
       const C *src = A.phat + (size_t)g * A.M + (size_t)line0 * n;
       for (int idx = tid; idx < (W << lgn); idx += nt) {
         const int c = idx >> lgn, j = idx & (n - 1);
-        sm[(size_t)j * RS + g * W + c] = (c < nl) ? src[idx] : zero;
+        sm[(size_t)geo_pad(A.geo, j) * RS + g * W + c] = (c < nl) ? src[idx] : zero;
       }
     }
     __syncthreads();
@@ -203,7 +203,7 @@ __global__ void __launch_bounds__(256, sizeof(T) == 4 ? 3 : 2) k_update(const __
     if (keepmask == 0) continue; /* the whole tile is masked: psix stays zero (zeroed at bind) */
     for (int idx = tid; idx < (n << lgW); idx += nt) {
       const int c = idx & (W - 1), s = idx >> lgW;
-      C *srow = sm + (size_t)s * RS + c;
+      C *srow = sm + (size_t)geo_pad(A.geo, s) * RS + c;
       C v = zero;
       if ((keepmask >> c) & 1u) {
         const int k = A.freq_of[s];
@@ -231,7 +231,7 @@ __global__ void __launch_bounds__(256, sizeof(T) == 4 ? 3 : 2) k_update(const __
     C *dst = A.psix + (size_t)f * A.M + (size_t)line0 * n;
     for (int idx = tid; idx < (W << lgn); idx += nt) {
       const int c = idx >> lgn, j = idx & (n - 1);
-      if ((keepmask >> c) & 1u) dst[idx] = sm[(size_t)j * RS + wb * W + c];
+      if ((keepmask >> c) & 1u) dst[idx] = sm[(size_t)geo_pad(A.geo, j) * RS + wb * W + c];
     }
     __syncthreads();
   }
@@ -261,7 +261,7 @@ __global__ void __launch_bounds__(256) k_rows(const __grid_constant__ Program P,
   const C zero = mk<C, T>((T)0, (T)0);
 
   /* zero, then Hermitian-extend the kept part of every factor: Z_k = A_k + i B_k (rows r, r+1) */
-  for (int idx = tid; idx < nx * RS; idx += nt) sm[idx] = zero;
+  for (int idx = tid; idx < A.geo.npad * RS; idx += nt) sm[idx] = zero;
   __syncthreads();
   for (int f = 0; f < P.nfac; ++f) {
     int cut = nxh; /* number of kept kx */
@@ -276,20 +276,35 @@ __global__ void __launch_bounds__(256) k_rows(const __grid_constant__ Program P,
       const C *p = src + (size_t)kx * A.R + 2 * c;
       C a = p[0], b = p[1];
       if (kx == 0 || 2 * kx == nx) { a.y = (T)0; b.y = (T)0; } /* C2R keeps the real part there */
-      sm[(size_t)kx * RS + f * Wc + c] = mk<C, T>(a.x - b.y, a.y + b.x);
-      if (kx > 0 && 2 * kx < nx) sm[(size_t)(nx - kx) * RS + f * Wc + c] = mk<C, T>(a.x + b.y, b.x - a.y);
+      sm[(size_t)geo_pad(A.geo, kx) * RS + f * Wc + c] = mk<C, T>(a.x - b.y, a.y + b.x);
+      if (kx > 0 && 2 * kx < nx) sm[(size_t)geo_pad(A.geo, nx - kx) * RS + f * Wc + c] = mk<C, T>(a.x + b.y, b.x - a.y);
     }
   }
   __syncthreads();
   if (P.nfac > 0) fft_dif<+1, T>(A.geo, sm, A.tw, P.nfac * Wc, RS);
+  T pc2 = (T)0, pc3 = (T)0, pc4 = (T)0;
+  if (P.rad_ok && P.ngrp == 1)
+    for (int t = P.grp[0].term_beg; t < P.grp[0].term_end; ++t) {
+      const T cf = (T)P.term[t].coef;
+      if (P.term[t].nf == 2) pc2 += cf;
+      else if (P.term[t].nf == 3) pc3 += cf;
+      else pc4 += cf;
+    }
   /* real-space products per group, forward transform, Hermitian split */
   for (int g = 0; g < P.ngrp; ++g) {
     const DGroup &G = P.grp[g];
     const int wb = (g == P.ngrp - 1) ? 0 : P.nfac;
     for (int idx = tid; idx < nx * Wc; idx += nt) {
       const int c = idx % Wc, s = idx / Wc;
-      const C *srow = sm + (size_t)s * RS + c;
+      const int sp = geo_pad(A.geo, s);
+      const C *srow = sm + (size_t)sp * RS + c;
       T pa = (T)0, pb = (T)0;
+      if (P.rad_ok) {
+        /* one factor field: sum_t coef_t r^nf_t = r^2 (c2 + r (c3 + r c4))  (Eq. 11 with one psi) */
+        const C v = srow[0];
+        pa = v.x * v.x * (pc2 + v.x * (pc3 + v.x * pc4));
+        pb = v.y * v.y * (pc2 + v.y * (pc3 + v.y * pc4));
+      } else
       for (int t = G.term_beg; t < G.term_end; ++t) {
         const DTerm &tm = P.term[t];
         T ta = (T)tm.coef, tb = (T)tm.coef;
@@ -301,15 +316,15 @@ __global__ void __launch_bounds__(256) k_rows(const __grid_constant__ Program P,
         pa += ta;
         pb += tb;
       }
-      sm[(size_t)s * RS + wb * Wc + c] = mk<C, T>(pa, pb);
+      sm[(size_t)sp * RS + wb * Wc + c] = mk<C, T>(pa, pb);
     }
     __syncthreads();
     fft_dit<-1, T>(A.geo, sm + wb * Wc, A.tw, Wc, RS);
     C *dst = A.phat + (size_t)g * A.M + r0;
     for (int idx = tid; idx < nxh * Wc; idx += nt) {
       const int c = idx % Wc, kx = idx / Wc;
-      const C z = sm[(size_t)kx * RS + wb * Wc + c];
-      const C zm = sm[(size_t)((nx - kx) & (nx - 1)) * RS + wb * Wc + c];
+      const C z = sm[(size_t)geo_pad(A.geo, kx) * RS + wb * Wc + c];
+      const C zm = sm[(size_t)geo_pad(A.geo, (nx - kx) & (nx - 1)) * RS + wb * Wc + c];
       const T h = (T)0.5;
       C *p = dst + (size_t)kx * A.R + 2 * c;
       p[0] = mk<C, T>(h * (z.x + zm.x), h * (z.y - zm.y));
@@ -347,13 +362,13 @@ template <int SGN, typename T> __global__ void __launch_bounds__(256) k_mid(cons
     const int c = idx % W, j = idx / W;
     int a = signed_index(j, ny);
     a = a < 0 ? -a : a;
-    sm[idx] = (nn && nn * a >= ny) ? mk<C, T>((T)0, (T)0) : base[(size_t)j * A.nz + c];
+    sm[geo_pad(A.geo, j) * W + c] = (nn && nn * a >= ny) ? mk<C, T>((T)0, (T)0) : base[(size_t)j * A.nz + c];
   }
   __syncthreads();
   fft_dif<SGN, T>(A.geo, sm, A.tw, W, W);
   for (int idx = threadIdx.x; idx < ny * W; idx += blockDim.x) {
     const int c = idx % W, s = idx / W;
-    base[(size_t)geo_rev(A.geo, s) * A.nz + c] = sm[idx];
+    base[(size_t)geo_rev(A.geo, s) * A.nz + c] = sm[geo_pad(A.geo, s) * W + c];
   }
 }
 
@@ -371,10 +386,10 @@ template <int SGN, typename T> __global__ void __launch_bounds__(256) k_last(con
   C *sm = reinterpret_cast<C *>(smem_raw);
   const int n = A.n;
   C *base = A.arr + (size_t)blockIdx.x * n;
-  for (int j = threadIdx.x; j < n; j += blockDim.x) sm[j] = base[j];
+  for (int j = threadIdx.x; j < n; j += blockDim.x) sm[geo_pad(A.geo, j)] = base[j];
   __syncthreads();
   fft_dif<SGN, T>(A.geo, sm, A.tw, 1, 1);
-  for (int j = threadIdx.x; j < n; j += blockDim.x) base[j] = sm[geo_slot(A.geo, j)];
+  for (int j = threadIdx.x; j < n; j += blockDim.x) base[j] = sm[geo_pad(A.geo, geo_slot(A.geo, j))];
 }
 
 /* ------------------------------------------------------------------------------------------ */
@@ -400,12 +415,12 @@ template <int DIR, typename T> __global__ void __launch_bounds__(256) k_user_x(c
   const long long ib = A.single ? ia : (rb % A.ny) * A.nz + rb / A.ny;
   if (DIR < 0) {
     for (int x = threadIdx.x; x < nx; x += blockDim.x)
-      sm[x] = mk<C, T>(A.real[ra * nx + x], A.single ? (T)0 : A.real[rb * nx + x]);
+      sm[geo_pad(A.geo, x)] = mk<C, T>(A.real[ra * nx + x], A.single ? (T)0 : A.real[rb * nx + x]);
     __syncthreads();
     fft_dif<-1, T>(A.geo, sm, A.tw, 1, 1);
     for (int kx = threadIdx.x; kx < nxh; kx += blockDim.x) {
-      const C z = sm[geo_slot(A.geo, kx)];
-      const C zm = sm[geo_slot(A.geo, (nx - kx) & (nx - 1))];
+      const C z = sm[geo_pad(A.geo, geo_slot(A.geo, kx))];
+      const C zm = sm[geo_pad(A.geo, geo_slot(A.geo, (nx - kx) & (nx - 1)))];
       const T h = (T)0.5;
       A.arr[(size_t)kx * R + ia] = mk<C, T>(h * (z.x + zm.x), h * (z.y - zm.y));
       if (!A.single) A.arr[(size_t)kx * R + ib] = mk<C, T>(h * (z.y + zm.y), h * (zm.x - z.x));
@@ -415,14 +430,14 @@ template <int DIR, typename T> __global__ void __launch_bounds__(256) k_user_x(c
       C a = A.arr[(size_t)kx * R + ia];
       C b = A.single ? mk<C, T>((T)0, (T)0) : A.arr[(size_t)kx * R + ib];
       if (kx == 0 || 2 * kx == nx) { a.y = (T)0; b.y = (T)0; }
-      sm[kx] = mk<C, T>(a.x - b.y, a.y + b.x);
-      if (kx > 0 && 2 * kx < nx) sm[nx - kx] = mk<C, T>(a.x + b.y, b.x - a.y);
+      sm[geo_pad(A.geo, kx)] = mk<C, T>(a.x - b.y, a.y + b.x);
+      if (kx > 0 && 2 * kx < nx) sm[geo_pad(A.geo, nx - kx)] = mk<C, T>(a.x + b.y, b.x - a.y);
     }
     __syncthreads();
     fft_dif<+1, T>(A.geo, sm, A.tw, 1, 1);
     const T sc = (T)A.scale;
     for (int x = threadIdx.x; x < nx; x += blockDim.x) {
-      const C z = sm[geo_slot(A.geo, x)];
+      const C z = sm[geo_pad(A.geo, geo_slot(A.geo, x))];
       A.real[ra * nx + x] = z.x * sc;
       if (!A.single) A.real[rb * nx + x] = z.y * sc;
     }
@@ -483,7 +498,7 @@ __global__ void __launch_bounds__(256) k_step1d(const __grid_constant__ Program 
   const C zero = mk<C, T>((T)0, (T)0);
   for (long long st = 0; st < A.nsteps; ++st) {
     /* steps 1-3: factor operators, mask, C2R (imaginary row unused) */
-    for (int idx = tid; idx < nx * RS; idx += nt) sm[idx] = zero;
+    for (int idx = tid; idx < A.geo.npad * RS; idx += nt) sm[idx] = zero;
     __syncthreads();
     for (int kx = tid; kx < nxh; kx += nt) {
       const ModeQ<T> mq = make_mode<T>(P, kx, 0, 0);
@@ -498,15 +513,15 @@ __global__ void __launch_bounds__(256) k_step1d(const __grid_constant__ Program 
         v.x *= (T)P.invN;
         v.y *= (T)P.invN;
         if (kx == 0 || 2 * kx == nx) v.y = (T)0;
-        sm[(size_t)kx * RS + f] = v;
-        if (kx > 0 && 2 * kx < nx) sm[(size_t)(nx - kx) * RS + f] = mk<C, T>(v.x, -v.y);
+        sm[(size_t)geo_pad(A.geo, kx) * RS + f] = v;
+        if (kx > 0 && 2 * kx < nx) sm[(size_t)geo_pad(A.geo, nx - kx) * RS + f] = mk<C, T>(v.x, -v.y);
       }
     }
     __syncthreads();
     if (P.nfac > 0) fft_dif<+1, T>(A.geo, sm, A.tw, P.nfac, RS);
     /* steps 3-4: products and R2C */
     for (int idx = tid; idx < nx; idx += nt) {
-      C *srow = sm + (size_t)idx * RS;
+      C *srow = sm + (size_t)geo_pad(A.geo, idx) * RS;
       for (int g = 0; g < P.ngrp; ++g) {
         const DGroup &G = P.grp[g];
         T pa = (T)0;
@@ -524,7 +539,7 @@ __global__ void __launch_bounds__(256) k_step1d(const __grid_constant__ Program 
     /* steps 5-6: noise and Eq. 18 */
     for (int kx = tid; kx < nxh; kx += nt) {
       const ModeQ<T> mq = make_mode<T>(P, kx, 0, 0);
-      const C *srow = sm + (size_t)kx * RS + P.nfac;
+      const C *srow = sm + (size_t)geo_pad(A.geo, kx) * RS + P.nfac;
       C phi[PSS_P_MAX_DYN], out[PSS_P_MAX_DYN];
 #pragma unroll
       for (int i = 0; i < PSS_P_MAX_DYN; ++i) phi[i] = (i < P.ndyn) ? A.state[(size_t)i * A.M + kx] : zero;

@@ -93,6 +93,12 @@ struct Geo {
   int32_t n;
   int32_t nr;
   int32_t lg[4]; /* log2 of the radices, first DIF pass first */
+  /* shared-memory padding against bank conflicts: slot p lives at row geo_pad(p) = p + sum_i (p >> sh[i]), one pad
+   * row per digit boundary of the slot index (unused entries are 31), so that every digit of the slot index maps to
+   * an ODD row stride: the stride-1 legs of the last pass and the digit-reversed accesses of the pointwise stages
+   * both spread over the banks.  npad = geo_pad(n-1) + 1 rows are allocated. */
+  int32_t sh[3];
+  int32_t npad;
 };
 
 #endif
