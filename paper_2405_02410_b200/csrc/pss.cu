@@ -435,6 +435,7 @@ int make_plan(pss_system *s) {
     }
     Wc = env_int("PSS_ROW_WC", Wc);
     if (Wc < 1) Wc = 1;
+    while (Wc & (Wc - 1)) Wc &= Wc - 1; /* a power of two (the kernel indexes with shifts) */
     while (Wc > 1 && (per * Wc > SMEM_MAX || 2 * Wc > R || R % (2 * Wc) != 0)) Wc >>= 1;
     pl.row_Wc = Wc;
     pl.row_smem = per * Wc;

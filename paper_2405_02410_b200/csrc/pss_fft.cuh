@@ -133,9 +133,11 @@ __device__ __forceinline__ void fft_pass(const Geo &g, typename cplx_of<T>::type
   const int nb = (1 << (lgn - LGR));   /* butterflies per column     */
   const int total = nb * ncol;
   const int ls = rs * geo_stride(g, lgLs); /* padded leg stride */
+  const bool notw = (lgLs == 0);                       /* every twiddle of this pass is w^0 = 1 */
+  const int lgc = (ncol & (ncol - 1)) ? -1 : (31 - __clz(ncol)); /* ncol a power of two: shifts */
   for (int idx = threadIdx.x; idx < total; idx += blockDim.x) {
-    const int c = idx % ncol;
-    const int b = idx / ncol;
+    const int c = (lgc >= 0) ? (idx & (ncol - 1)) : (idx % ncol);
+    const int b = (lgc >= 0) ? (idx >> lgc) : (idx / ncol);
     const int i = b & ((1 << lgLs) - 1);
     const int blk = b >> lgLs;
     C *p = buf + (size_t)geo_pad(g, (blk << lgL) + i) * rs + c;
@@ -143,7 +145,7 @@ __device__ __forceinline__ void fft_pass(const Geo &g, typename cplx_of<T>::type
     C v[R];
 #pragma unroll
     for (int k = 0; k < R; ++k) v[k] = p[k * ls];
-    if (DIT) {
+    if (DIT && !notw) {
 #pragma unroll
       for (int m = 1; m < R; ++m) {
         const C w = __ldg(tw + m * tws);
@@ -151,7 +153,7 @@ __device__ __forceinline__ void fft_pass(const Geo &g, typename cplx_of<T>::type
       }
     }
     dft_reg<LGR, SGN>(v);
-    if (!DIT) {
+    if (!DIT && !notw) {
 #pragma unroll
       for (int m = 1; m < R; ++m) {
         const C w = __ldg(tw + m * tws);

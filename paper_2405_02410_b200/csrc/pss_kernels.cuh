@@ -136,8 +136,7 @@ __global__ void __launch_bounds__(256, sizeof(T) == 4 ? 3 : 2) k_update(const __
         } else {
           srow[0] = phi;
         }
-        continue;
-      }
+      } else {
       C phi[PSS_P_MAX_DYN];
 #pragma unroll
       for (int i = 0; i < PSS_P_MAX_DYN; ++i) phi[i] = (i < P.ndyn) ? A.state[(size_t)i * A.M + gi] : zero;
@@ -179,6 +178,7 @@ __global__ void __launch_bounds__(256, sizeof(T) == 4 ? 3 : 2) k_update(const __
 #pragma unroll
         for (int i = 0; i < PSS_P_MAX_DYN; ++i)
           if (i < P.ndyn) srow[i * W] = phi[i];
+      }
       }
     }
   }
@@ -254,7 +254,7 @@ __global__ void __launch_bounds__(256) k_rows(const __grid_constant__ Program P,
   typedef typename cplx_of<T>::type C;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   C *sm = reinterpret_cast<C *>(smem_raw);
-  const int nx = A.nx, nxh = nx / 2 + 1, Wc = A.Wc;
+  const int nx = A.nx, nxh = nx / 2 + 1, Wc = A.Wc, lgWc = 31 - __clz(Wc); /* Wc is a power of two */
   const int RS = (P.nfac + (P.ngrp > 1 ? 1 : 0)) * Wc;
   const long long r0 = (long long)blockIdx.x * (2 * Wc);
   const int tid = threadIdx.x, nt = blockDim.x;
@@ -272,7 +272,7 @@ __global__ void __launch_bounds__(256) k_rows(const __grid_constant__ Program P,
     }
     const C *src = A.psix + (size_t)f * A.M + r0;
     for (int idx = tid; idx < cut * Wc; idx += nt) {
-      const int c = idx % Wc, kx = idx / Wc;
+      const int c = idx & (Wc - 1), kx = idx >> lgWc;
       const C *p = src + (size_t)kx * A.R + 2 * c;
       C a = p[0], b = p[1];
       if (kx == 0 || 2 * kx == nx) { a.y = (T)0; b.y = (T)0; } /* C2R keeps the real part there */
@@ -295,7 +295,7 @@ __global__ void __launch_bounds__(256) k_rows(const __grid_constant__ Program P,
     const DGroup &G = P.grp[g];
     const int wb = (g == P.ngrp - 1) ? 0 : P.nfac;
     for (int idx = tid; idx < nx * Wc; idx += nt) {
-      const int c = idx % Wc, s = idx / Wc;
+      const int c = idx & (Wc - 1), s = idx >> lgWc;
       const int sp = geo_pad(A.geo, s);
       const C *srow = sm + (size_t)sp * RS + c;
       T pa = (T)0, pb = (T)0;
@@ -322,7 +322,7 @@ __global__ void __launch_bounds__(256) k_rows(const __grid_constant__ Program P,
     fft_dit<-1, T>(A.geo, sm + wb * Wc, A.tw, Wc, RS);
     C *dst = A.phat + (size_t)g * A.M + r0;
     for (int idx = tid; idx < nxh * Wc; idx += nt) {
-      const int c = idx % Wc, kx = idx / Wc;
+      const int c = idx & (Wc - 1), kx = idx >> lgWc;
       const C z = sm[(size_t)geo_pad(A.geo, kx) * RS + wb * Wc + c];
       const C zm = sm[(size_t)geo_pad(A.geo, (nx - kx) & (nx - 1)) * RS + wb * Wc + c];
       const T h = (T)0.5;
