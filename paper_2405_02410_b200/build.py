@@ -30,7 +30,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if force or needs_build():
         nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
         tmp = LIB + ".tmp.%d" % os.getpid()
-        cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-I", INCLUDE, "-o", tmp] + SOURCES
+        cmd = [nvcc] + NVCC_FLAGS + os.environ.get("PSS_NVCC_EXTRA", "").split() + (["-Xptxas", "-v"] if verbose else []) + ["-I", INCLUDE, "-o", tmp] + SOURCES
         subprocess.run(cmd, check=True, cwd=CSRC)
         os.replace(tmp, LIB)
     return LIB

@@ -45,7 +45,7 @@ constexpr int THREADS = TT + NT;
 constexpr int NCTA = 129;             /* 128 CTAs own 4 packed rows + 4 columns; CTA 128 owns column kx = 512 */
 constexpr int PITCH = 65;             /* k1-row pitch of an exchange buffer (float2)       */
 constexpr int BUF = 16 * PITCH + 4;   /* one line's exchange buffer; = 4 mod 16            */
-constexpr size_t SMEM_BYTES = (size_t)(16 * 64 + 64 + 4 * BUF + 2 * 16 * TT) * sizeof(float2) + (size_t)16 * TT * sizeof(float4);
+constexpr size_t SMEM_BYTES = (size_t)(4 * BUF + 2 * 16 * TT) * sizeof(float2) + (size_t)16 * TT * sizeof(float4);
 
 typedef f2d::Args Args;
 
@@ -72,9 +72,9 @@ __device__ __forceinline__ void dft4(float2 &x0, float2 &x1, float2 &x2, float2 
 }
 
 struct Lane {
-  float2 *xl;       /* this line's exchange buffer                         */
-  const float2 *t1; /* T1 + tq            : T1[k1*64 + tq] = w1024^(k1 tq) */
-  const float2 *t2; /* T2 + (tq & 3)      : T2[k2*4 + n3]  = w64^(k2 n3)   */
+  float2 *xl;       /* this line's exchange buffer                 */
+  float2 t1[16];    /* t1[k1] = w1024^(k1 tq)   (registers)        */
+  float2 t2[16];    /* t2[k2] = w64^(k2 (tq & 3))                  */
   int tq;
 };
 
@@ -84,7 +84,7 @@ __device__ __forceinline__ void fwd_dif(float2 (&v)[16], const Lane &ln) {
 #pragma unroll
   for (int k1 = 0; k1 < 16; ++k1) {
     float2 x = v[k1];
-    if (k1 > 0) x = cmulf(x, ln.t1[k1 * 64]);
+    if (k1 > 0) x = cmulf(x, ln.t1[k1]);
     ln.xl[k1 * PITCH + ln.tq] = x;
   }
   tsync();
@@ -95,7 +95,7 @@ __device__ __forceinline__ void fwd_dif(float2 (&v)[16], const Lane &ln) {
 #pragma unroll
   for (int k2 = 0; k2 < 16; ++k2) {
     float2 x = v[k2];
-    if (k2 > 0) x = cmulf(x, ln.t2[k2 * 4]);
+    if (k2 > 0) x = cmulf(x, ln.t2[k2]);
     base[4 * k2] = x;
   }
   tsync();
@@ -122,7 +122,7 @@ __device__ __forceinline__ void fwd_dit(float2 (&v)[16], const Lane &ln) {
 #pragma unroll
   for (int k2 = 0; k2 < 16; ++k2) {
     float2 x = base[4 * k2];
-    if (k2 > 0) x = cmulf(x, ln.t2[k2 * 4]);
+    if (k2 > 0) x = cmulf(x, ln.t2[k2]);
     v[k2] = x;
   }
   dft_reg<4, -1>(v);
@@ -132,7 +132,7 @@ __device__ __forceinline__ void fwd_dit(float2 (&v)[16], const Lane &ln) {
 #pragma unroll
   for (int k1 = 0; k1 < 16; ++k1) {
     float2 x = ln.xl[k1 * PITCH + ln.tq];
-    if (k1 > 0) x = cmulf(x, ln.t1[k1 * 64]);
+    if (k1 > 0) x = cmulf(x, ln.t1[k1]);
     v[k1] = x;
   }
   dft_reg<4, -1>(v);
@@ -144,7 +144,7 @@ __device__ __forceinline__ void fwd_dit(float2 (&v)[16], const Lane &ln) {
  * barrier is read with ld.global.cg. */
 __device__ __forceinline__ void grid_barrier(unsigned long long *ctr, unsigned long long target, int dbg) {
   tsync();
-  if (threadIdx.x == 0) {
+  if ((threadIdx.x & (TT - 1)) == 0) {
     asm volatile("red.release.gpu.global.add.u64 [%0], 1;" ::"l"(ctr) : "memory");
     if (!(dbg & 1)) {
       unsigned long long v;
@@ -158,9 +158,7 @@ __device__ __forceinline__ void grid_barrier(unsigned long long *ctr, unsigned l
 template <bool PRUNE>
 __global__ void __launch_bounds__(THREADS, 1) k_fused2d_v2(const __grid_constant__ Program P, const Args A) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  float2 *T1 = reinterpret_cast<float2 *>(smem_raw);           /* [16][64]                                  */
-  float2 *T2 = T1 + 16 * 64;                                   /* [16][4]                                   */
-  float2 *xs = T2 + 64;                                        /* [4][BUF] exchange buffers                 */
+  float2 *xs = reinterpret_cast<float2 *>(smem_raw);           /* [4][BUF] exchange buffers                 */
   float2 *zbuf = xs + 4 * BUF;                                 /* [2][16 r][256 tid] unit noise z           */
   float4 *tab = reinterpret_cast<float4 *>(zbuf + 2 * 16 * TT); /* [16 r][256 tid] per-mode coefficients     */
 
@@ -181,6 +179,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_fused2d_v2(const __grid_constant
   const long long nphase = A.nsteps + (A.prologue ? 1 : 0);
 
   if (noisew) {
+    asm volatile("setmaxnreg.dec.sync.aligned.u32 64;"); /* hand registers to the transform warps */
     /* ============ noise warps: z(step s+1) is drawn while the transform warps work on step s ============ */
     if (!noisy || A.nsteps <= 0) return;
     NoiseKey K;
@@ -205,16 +204,17 @@ __global__ void __launch_bounds__(THREADS, 1) k_fused2d_v2(const __grid_constant
   }
 
   /* ================= transform warps ================= */
+  asm volatile("setmaxnreg.inc.sync.aligned.u32 184;"); /* 8 x 32 x (64 + 184) = 63488 <= 65536 registers */
   const bool need_inv = colw && keep_axis(P.dealias, P.fac[0].order, kx, N);
   const bool roww = b < 128;
   Lane ln;
   ln.xl = xs + L * BUF;
-  ln.t1 = T1 + tq;
-  ln.t2 = T2 + (tq & 3);
   ln.tq = tq;
-
-  for (int i = tid; i < 16 * 64; i += TT) T1[i] = A.tw[((i >> 6) * (i & 63)) & (N - 1)];
-  if (tid < 64) T2[tid] = A.tw[(16 * (tid >> 2) * (tid & 3)) & (N - 1)];
+#pragma unroll
+  for (int i = 0; i < 16; ++i) {
+    ln.t1[i] = A.tw[(i * tq) & (N - 1)];
+    ln.t2[i] = A.tw[(16 * i * (tq & 3)) & (N - 1)];
+  }
 
   /* per-mode coefficients: (dt*outer, 1/(1 - dt L), noise amplitude, factor op * mask / N), and the state */
   float2 st[16];
