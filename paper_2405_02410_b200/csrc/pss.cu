@@ -17,7 +17,6 @@
 
 #include "pss_kernels.cuh"
 #include "pss_fused2d.cuh"
-#include "pss_fused2d_v2.cuh"
 
 namespace {
 
@@ -40,8 +39,7 @@ struct Plan {
   int mid_W, mid_threads; size_t mid_smem;
   int one_threads; size_t one_smem; /* 1D */
   int kx_keep_max;                  /* max over factors of the number of kept kx */
-  int fused;                        /* persistent 1024^2 fp32 kernel runs the steps: 2 = pss_fused2d_v2.cuh (default),
-                                       1 = pss_fused2d.cuh (PSS_FUSED=1), 0 = generic two-kernel path (PSS_FUSED=0) */
+  int fused;                        /* 1: the persistent 1024^2 fp32 kernel of pss_fused2d.cuh runs the steps (PSS_FUSED=0 disables) */
   int fused_prune;                  /* its input-pruned instantiation (mask cutoff <= n/4 on both axes)       */
 };
 
@@ -382,7 +380,7 @@ int make_plan(pss_system *s) {
     }
     if (cut > pl.kx_keep_max) pl.kx_keep_max = cut;
   }
-  pl.fused = fused2d_eligible(s) ? (env_int("PSS_FUSED", 2) == 1 ? 1 : 2) : 0;
+  pl.fused = fused2d_eligible(s) ? 1 : 0;
   if (pl.fused) {
     const int nn = (P.dealias == PSS_DEALIAS_OFF) ? 1 : ((P.dealias == PSS_DEALIAS_TWO_THIRDS ? 2 : P.fac[0].order) + 1);
     pl.fused_prune = (nn >= 4) ? 1 : 0;
@@ -467,7 +465,7 @@ void carve_workspace(pss_system *s) {
   s->off_ureal = off; off += align_up((size_t)s->N * s->rsize, 256);
   for (int j = 0; j < 3; ++j) { s->off_tw[j] = off; off += align_up((size_t)s->n[j] * s->csize, 256); }
   s->off_rev = off; off += align_up((size_t)2 * (size_t)s->n[s->ndim - 1] * sizeof(unsigned short), 256);
-  s->off_bar = off; off += 1024; /* v1: one 64-bit counter; v2: one 32-bit epoch flag per CTA */
+  s->off_bar = off; off += 256;
   s->ws_need = off;
 }
 
@@ -504,25 +502,13 @@ int setup_fused(pss_system *s) {
   CK(cudaGetDevice(&dev));
   CK(cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev));
   CK(cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev));
-  int ncta = 0;
-  if (s->plan.fused == 2) {
-    CK(cudaFuncSetAttribute(f2e::k_fused2d_v2<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)f2e::SMEM_BYTES));
-    CK(cudaFuncSetAttribute(f2e::k_fused2d_v2<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)f2e::SMEM_BYTES));
-    if (s->plan.fused_prune)
-      CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, f2e::k_fused2d_v2<true>, f2e::THREADS, f2e::SMEM_BYTES));
-    else
-      CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, f2e::k_fused2d_v2<false>, f2e::THREADS, f2e::SMEM_BYTES));
-    ncta = f2e::NCTA;
-  } else {
-    CK(cudaFuncSetAttribute(f2d::k_fused2d<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)f2d::SMEM_BYTES));
-    CK(cudaFuncSetAttribute(f2d::k_fused2d<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)f2d::SMEM_BYTES));
-    if (s->plan.fused_prune)
-      CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, f2d::k_fused2d<true>, f2d::THREADS, f2d::SMEM_BYTES));
-    else
-      CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, f2d::k_fused2d<false>, f2d::THREADS, f2d::SMEM_BYTES));
-    ncta = f2d::NCTA;
-  }
-  if (!coop || (long long)occ * nsm < ncta) s->plan.fused = 0;
+  CK(cudaFuncSetAttribute(f2d::k_fused2d<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)f2d::SMEM_BYTES));
+  CK(cudaFuncSetAttribute(f2d::k_fused2d<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)f2d::SMEM_BYTES));
+  if (s->plan.fused_prune)
+    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, f2d::k_fused2d<true>, f2d::THREADS, f2d::SMEM_BYTES));
+  else
+    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, f2d::k_fused2d<false>, f2d::THREADS, f2d::SMEM_BYTES));
+  if (!coop || (long long)occ * nsm < f2d::NCTA) s->plan.fused = 0;
   return PSS_OK;
 }
 
@@ -655,14 +641,10 @@ int launch_fused(pss_system *s, int64_t nsteps) {
   a.nsteps = nsteps;
   a.step0 = s->step;
   a.prologue = s->psix_valid ? 0 : 1;
-  a.dbg = env_int("PSS_DBG", 0);
   void *params[2] = {(void *)&s->P, (void *)&a};
-  const bool v2 = s->plan.fused == 2;
-  const void *fn = v2 ? (s->plan.fused_prune ? (const void *)f2e::k_fused2d_v2<true> : (const void *)f2e::k_fused2d_v2<false>)
-                      : (s->plan.fused_prune ? (const void *)f2d::k_fused2d<true> : (const void *)f2d::k_fused2d<false>);
+  const void *fn = s->plan.fused_prune ? (const void *)f2d::k_fused2d<true> : (const void *)f2d::k_fused2d<false>;
   prof_mark(s, KIND_FUSED, true);
-  cudaError_t e = cudaLaunchCooperativeKernel(fn, dim3(f2d::NCTA), dim3(v2 ? f2e::THREADS : f2d::THREADS), params,
-                                              v2 ? f2e::SMEM_BYTES : f2d::SMEM_BYTES, s->stream);
+  cudaError_t e = cudaLaunchCooperativeKernel(fn, dim3(f2d::NCTA), dim3(f2d::THREADS), params, f2d::SMEM_BYTES, s->stream);
   prof_mark(s, KIND_FUSED, false);
   if (e != cudaSuccess) return cuda_fail(s, e, "k_fused2d");
   CKL("k_fused2d");
