@@ -5,7 +5,7 @@
     python bench.py --impl reference ...            # the CPU oracle, timed on the host cores
 
 One bench "step" is one call pss_step(inner): `inner` consecutive time steps of the whole hot path
-(k_rows + k_update per time step) on the workload's lattice.  The state of a time stepper is consumed by
+(k_rows + k_update per time step, or all of them inside one persistent k_fused2d launch at 1024^2 fp32) on the workload's lattice.  The state of a time stepper is consumed by
 the next time step, so inside one bench step the working set is as warm as the workload makes it; BETWEEN
 timed bench steps L2 is flushed (a 256 MiB buffer is written), so every timed step starts cold.
 
@@ -280,7 +280,7 @@ def main():
                     "h2d_bytes_per_step": len(dyn_names) * S, "d2h_bytes_per_step": len(dyn_names) * S,
                     "note": "pss_set_field(host) + pss_step(%d) + pss_get_field(host) per bench step" % inner},
             "roofline": {"bound": "hbm", "kernel": dom, "achieved": ach, "peak": peak, "unit": "GB/s",
-                         "frac": ach / peak, "traffic": ncu_traffic(dom), "peak_source": peak_src,
+                         "frac": ach / peak, "traffic": ncu_traffic(args.workload, dom), "peak_source": peak_src,
                          "algorithmic_bytes_per_launch": kb[dom], "launch_ms": dom_ms,
                          "timesteps_per_launch": prof_n if dom == "k_fused2d" else 1,
                          "kernel_ms": {k: v[0] for k, v in prof.items() if v[1] > 0},
@@ -320,14 +320,20 @@ def kernel_bytes(cfg, S, g, steps_per_fused_launch):
     return {"k_rows": rows, "k_update": upd, "k_mid": mid, "k_fused2d": total * steps_per_fused_launch}
 
 
-def ncu_traffic(kernel):
-    """dram bytes per launch of the kernel from the committed ncu capture (profiles/), or None."""
-    p = os.path.join(ROOT, "profiles", "ncu_traffic.json")
+def ncu_traffic(workload, kernel):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel` on `workload` from the committed
+    ncu --set full capture (profiles/ncu_traffic.csv), or None.  For k_fused2d one launch of that capture ran
+    `timesteps_per_launch` time steps (the working set is L2-resident: DRAM traffic is mostly the first touch)."""
+    p = os.path.join(ROOT, "profiles", "ncu_traffic.csv")
     try:
         with open(p) as f:
-            return json.load(f).get(kernel)
+            for ln in f.read().splitlines()[1:]:
+                w, k, b, n, src = ln.split(",")
+                if w == workload and k == kernel:
+                    return {"dram_bytes_per_launch": int(b), "timesteps_per_launch": int(n), "source": src}
     except Exception:
-        return None
+        pass
+    return None
 
 
 if __name__ == "__main__":
