@@ -150,6 +150,7 @@ def main():
     ap.add_argument("--ref-budget", type=float, default=20.0, help="seconds of oracle work for the reference arm")
     ap.add_argument("--cpu-budget", type=float, default=12.0, help="seconds of oracle work for cpu_baseline")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-compare", action="store_true", help="skip the cuFFT+cuRAND comparison step (2D Model B only)")
     args = ap.parse_args()
 
     rank = int(os.environ.get("RANK", "0"))
@@ -295,9 +296,33 @@ def main():
             r, n, el, cores = oracle_rate(cfg, args.prec, args.cpu_budget, 64)
             line["cpu_baseline"] = {"value": r, "unit": "timesteps/s", "cores": cores, "kind": "oracle",
                                     "sample": "%d oracle time steps of %s after 1 warm-up step, %.1f s" % (n, args.workload, el)}
+        if not args.no_compare and world == 1 and cfg["model"] == "model_b" and len(cfg["n"]) == 2 and args.prec == "f32":
+            line["cufft_curand_comparison"] = cufft_compare(cfg)
         print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
+
+
+def cufft_compare(cfg):
+    """The same 2D Model-B step built the way the paper describes its GPU path (cuFFT for every transform, cuRAND
+    noise, one pointwise kernel per arrow; paper_2405_02410_b200/compare/cufft_modelb.cu), timed with CUDA events on
+    this GPU.  A comparison baseline only (north_star); the product never loads it."""
+    import ctypes
+    try:
+        from paper_2405_02410_b200 import build as pss_build
+        lib = ctypes.CDLL(pss_build.build_compare())
+        us = ctypes.c_double(0.0)
+        pr = cfg["params"]
+        nsteps = 200 if cfg["n"][0] <= 2048 else 30
+        rc = lib.cmp_cufft_modelb(int(cfg["n"][0]), int(cfg["n"][1]), ctypes.c_double(float(cfg["dx"])),
+                                  ctypes.c_double(cfg["dt"]), ctypes.c_double(pr["a"]), ctypes.c_double(pr["b"]),
+                                  ctypes.c_double(pr["k"]), ctypes.c_double(pr["D"]), nsteps, 20, ctypes.byref(us))
+        if rc != 0:
+            return {"unavailable": "cmp_cufft_modelb returned %d" % rc}
+        return {"us_per_timestep": us.value, "timesteps_per_s": 1e6 / us.value, "timed_steps": nsteps,
+                "what": "mask copy, cufftExecC2R, cube, cufftExecR2C, curandGenerateNormal, cufftExecR2C, Eq. 18 kernel"}
+    except Exception as e:  # the comparison is optional context, never a reason to fail the bench
+        return {"unavailable": repr(e)[:200]}
 
 
 def kernel_bytes(cfg, S, g, steps_per_fused_launch):
