@@ -63,7 +63,7 @@ struct pss_system {
   size_t csize, rsize;
   int64_t M, N; /* modes (half-spectrum), sites */
   /* workspace carve-up (byte offsets) */
-  size_t off_state, off_psix, off_phat, off_scratch, off_ureal, off_tw[3], off_rev, off_bar, ws_need;
+  size_t off_state, off_psix, off_phat, off_scratch, off_ureal, off_tw[3], off_bar, ws_need;
   unsigned long long bar_count; /* value of the fused kernel's grid-barrier counter */
   char *ws;
   cudaStream_t stream;
@@ -336,6 +336,17 @@ Geo make_geo(int64_t n) {
   for (int i = 0; i < 3; ++i) g.sh[i] = 31;
   for (int q = np - 1; q >= 1; --q) { b += g.lg[q]; g.sh[k++] = b; }
   g.npad = geo_pad_h(g, (int)n - 1) + 1;
+  /* digit fields: the first pass's digit is the LOW digit of the frequency and the HIGH digit of the slot */
+  int fs = 0, rem = lg;
+  for (int q = 0; q < 4; ++q) {
+    if (q < np) {
+      rem -= g.lg[q];
+      g.fs[q] = fs; g.ps[q] = rem; g.fm[q] = (1 << g.lg[q]) - 1;
+      fs += g.lg[q];
+    } else {
+      g.fs[q] = 0; g.ps[q] = 0; g.fm[q] = 0;
+    }
+  }
   return g;
 }
 
@@ -426,7 +437,8 @@ int make_plan(pss_system *s) {
     int Wc = 1;
     for (int cand = 8; cand >= 1; cand >>= 1) {
       if (2 * cand > R) continue;
-      if (per * cand > SMEM_SOFT && cand > 1) continue;
+      if (per * cand > SMEM_SOFT && cand > wc_sector) continue; /* whole 32-byte sectors first, then occupancy */
+      if (per * cand > SMEM_MAX) continue;
       if (R / (2 * cand) < 2 * 148 && cand > wc_sector) continue;
       Wc = cand;
       break;
@@ -438,7 +450,11 @@ int make_plan(pss_system *s) {
     pl.row_Wc = Wc;
     pl.row_smem = per * Wc;
     pl.row_blocks = (int)(R / (2 * Wc));
-    pl.row_threads = env_int("PSS_ROW_T", round_threads((nx / 8) * Wc * (P.nfac > 0 ? P.nfac : 1)));
+    pl.row_threads = round_threads((nx / 8) * Wc * (P.nfac > 0 ? P.nfac : 1));
+    /* a tile that leaves room for one CTA per SM only gets 512 threads (fp32; the fp64 butterflies need the registers) */
+    if (pl.row_smem > 113 * 1024 && cs == 8 && (nx / 16) * Wc * (P.nfac > 0 ? P.nfac : 1) >= 512) pl.row_threads = 512;
+    pl.row_threads = env_int("PSS_ROW_T", pl.row_threads);
+    if (pl.row_threads > 512) pl.row_threads = 512;
   }
   if (s->ndim == 3) {
     int W = (int)(128 / cs);
@@ -464,7 +480,6 @@ void carve_workspace(pss_system *s) {
   s->off_scratch = off; off += arr;
   s->off_ureal = off; off += align_up((size_t)s->N * s->rsize, 256);
   for (int j = 0; j < 3; ++j) { s->off_tw[j] = off; off += align_up((size_t)s->n[j] * s->csize, 256); }
-  s->off_rev = off; off += align_up((size_t)2 * (size_t)s->n[s->ndim - 1] * sizeof(unsigned short), 256);
   s->off_bar = off; off += 256;
   s->ws_need = off;
 }
@@ -483,7 +498,8 @@ template <typename T> const typename cplx_of<T>::type *twp(pss_system *s, int ax
 template <typename T> int set_attrs(pss_system *s) {
   CK(cudaFuncSetAttribute(k_update<T, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_MAX));
   CK(cudaFuncSetAttribute(k_update<T, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_MAX));
-  CK(cudaFuncSetAttribute(k_rows<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_MAX));
+  CK(cudaFuncSetAttribute(k_rows<T, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_MAX));
+  CK(cudaFuncSetAttribute(k_rows<T, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_MAX));
   CK(cudaFuncSetAttribute(k_mid<-1, T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_MAX));
   CK(cudaFuncSetAttribute(k_mid<+1, T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_MAX));
   CK(cudaFuncSetAttribute(k_last<-1, T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_MAX));
@@ -524,26 +540,6 @@ template <typename T> int upload_twiddles(pss_system *s) {
     }
     CK(cudaMemcpyAsync(s->ws + s->off_tw[j], tw.data(), tw.size() * sizeof(C), cudaMemcpyHostToDevice, s->stream));
     CK(cudaStreamSynchronize(s->stream)); /* tw is a stack-lifetime host buffer */
-  }
-  /* digit-reversal tables of the last axis (k_update): slot_of[k], freq_of[s] */
-  {
-    const Geo &g = s->plan.geo[s->ndim - 1];
-    const int n = g.n;
-    std::vector<unsigned short> tab((size_t)2 * n);
-    int lgn = 0;
-    for (int q = 0; q < g.nr; ++q) lgn += g.lg[q];
-    for (int f = 0; f < n; ++f) {
-      int p = 0, rem = lgn, ff = f;
-      for (int q = 0; q < g.nr; ++q) {
-        rem -= g.lg[q];
-        p |= (ff & ((1 << g.lg[q]) - 1)) << rem;
-        ff >>= g.lg[q];
-      }
-      tab[(size_t)f] = (unsigned short)geo_pad_h(g, p);
-      tab[(size_t)n + p] = (unsigned short)f;
-    }
-    CK(cudaMemcpyAsync(s->ws + s->off_rev, tab.data(), tab.size() * sizeof(unsigned short), cudaMemcpyHostToDevice, s->stream));
-    CK(cudaStreamSynchronize(s->stream));
   }
   return PSS_OK;
 }
@@ -589,8 +585,6 @@ template <typename T> int launch_update(pss_system *s, int prologue, uint64_t st
   a.psix = carr<T>(s, s->off_psix, 0);
   a.phat = carr<T>(s, s->off_phat, 0);
   a.tw = twp<T>(s, s->ndim - 1);
-  a.slot_of = reinterpret_cast<const unsigned short *>(s->ws + s->off_rev);
-  a.freq_of = a.slot_of + s->n[s->ndim - 1];
   a.M = arr_stride(s);
   a.n = (int)s->n[s->ndim - 1];
   a.lgn = ilog2(a.n);
@@ -622,7 +616,8 @@ template <typename T> int launch_rows(pss_system *s) {
   a.Wc = s->plan.row_Wc;
   a.geo = s->plan.geo[0];
   prof_mark(s, KIND_ROWS, true);
-  k_rows<T><<<s->plan.row_blocks, s->plan.row_threads, s->plan.row_smem, s->stream>>>(P, a);
+  if (s->plan.row_threads > 256) k_rows<T, true><<<s->plan.row_blocks, s->plan.row_threads, s->plan.row_smem, s->stream>>>(P, a);
+  else k_rows<T, false><<<s->plan.row_blocks, s->plan.row_threads, s->plan.row_smem, s->stream>>>(P, a);
   prof_mark(s, KIND_ROWS, false);
   CKL("k_rows");
   if (s->ndim == 3) return launch_mid<T>(s, -1, s->off_phat, P.ngrp, P.nxh);

@@ -121,6 +121,16 @@ __device__ __forceinline__ int geo_stride(const Geo &g, int lo) {
   return w;
 }
 
+/* branch-free digit reversal (same maps as geo_slot / geo_rev) */
+__device__ __forceinline__ int geo_slot_fast(const Geo &g, int f) {
+  return (((f >> g.fs[0]) & g.fm[0]) << g.ps[0]) | (((f >> g.fs[1]) & g.fm[1]) << g.ps[1]) |
+         (((f >> g.fs[2]) & g.fm[2]) << g.ps[2]) | (((f >> g.fs[3]) & g.fm[3]) << g.ps[3]);
+}
+__device__ __forceinline__ int geo_rev_fast(const Geo &g, int p) {
+  return (((p >> g.ps[0]) & g.fm[0]) << g.fs[0]) | (((p >> g.ps[1]) & g.fm[1]) << g.fs[1]) |
+         (((p >> g.ps[2]) & g.fm[2]) << g.fs[2]) | (((p >> g.ps[3]) & g.fm[3]) << g.fs[3]);
+}
+
 /* one radix-2^LGR pass over `ncol` interleaved columns: element (j, c) at buf[j*rs + c], c < ncol <= rs
  * (several buffers of W columns each sit side by side in one row of rs columns).  lgL = log2 of the current sub-length L, lgn = log2 n.
  * DIT = false: butterfly then twiddle (DIF).  DIT = true: twiddle then butterfly. */

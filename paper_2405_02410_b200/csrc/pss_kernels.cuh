@@ -24,8 +24,6 @@ template <typename T> struct UpdArgs {
   typename cplx_of<T>::type *psix;  /* [nfac][M] */
   typename cplx_of<T>::type *phat;  /* [ngrp][M] */
   const typename cplx_of<T>::type *tw;
-  const unsigned short *slot_of; /* slot_of[k]: PADDED shared-memory row of frequency k after fft_dif (digit reversal) */
-  const unsigned short *freq_of; /* freq_of[s]: frequency held by slot s                                        */
   long long M;
   int n, lgn;   /* last-axis length (a power of two) */
   int nlines;   /* nxh (2D) or nxh*ny (3D) */
@@ -94,6 +92,7 @@ __global__ void __launch_bounds__(256, sizeof(T) == 4 ? 3 : 2) k_update(const __
   if (!A.prologue && P.ngrp > 0) {
     for (int g = 0; g < P.ngrp; ++g) {
       const C *src = A.phat + (size_t)g * A.M + (size_t)line0 * n;
+#pragma unroll 4
       for (int idx = tid; idx < (W << lgn); idx += nt) {
         const int c = idx >> lgn, j = idx & (n - 1);
         sm[(size_t)geo_pad(A.geo, j) * RS + g * W + c] = (c < nl) ? src[idx] : zero;
@@ -106,8 +105,9 @@ __global__ void __launch_bounds__(256, sizeof(T) == 4 ? 3 : 2) k_update(const __
   for (int c = 0; c < nl; ++c) {
     const int line = line0 + c;
     const LineQ<T> lq = make_line<T>(P, line, A.lg_ny);
+#pragma unroll 2
     for (int k = tid; k < n; k += nt) {
-      C *srow = sm + (size_t)A.slot_of[k] * RS + c;
+      C *srow = sm + (size_t)geo_pad(A.geo, geo_slot_fast(A.geo, k)) * RS + c;
       const size_t gi = (size_t)line * n + k;
       if (RAD) {
         const C phi = A.state[gi];
@@ -206,7 +206,7 @@ __global__ void __launch_bounds__(256, sizeof(T) == 4 ? 3 : 2) k_update(const __
       C *srow = sm + (size_t)geo_pad(A.geo, s) * RS + c;
       C v = zero;
       if ((keepmask >> c) & 1u) {
-        const int k = A.freq_of[s];
+        const int k = geo_rev_fast(A.geo, s);
         if (keep_axis(P.dealias, F.order, k, n)) {
           const LineQ<T> lq = make_line<T>(P, line0 + c, A.lg_ny);
           const ModeQ<T> mq = line_mode<T>(P, lq, k, n, qs_last);
@@ -229,6 +229,7 @@ __global__ void __launch_bounds__(256, sizeof(T) == 4 ? 3 : 2) k_update(const __
     __syncthreads();
     fft_dit<+1, T>(A.geo, sm + wb * W, A.tw, W, RS);
     C *dst = A.psix + (size_t)f * A.M + (size_t)line0 * n;
+#pragma unroll 4
     for (int idx = tid; idx < (W << lgn); idx += nt) {
       const int c = idx >> lgn, j = idx & (n - 1);
       if ((keepmask >> c) & 1u) dst[idx] = sm[(size_t)geo_pad(A.geo, j) * RS + wb * W + c];
@@ -249,8 +250,9 @@ template <typename T> struct RowArgs {
   Geo geo;
 };
 
-template <typename T>
-__global__ void __launch_bounds__(256) k_rows(const __grid_constant__ Program P, const RowArgs<T> A) {
+/* BIG: one CTA per SM (tile > half of the shared memory): 512 threads, else 256 threads and 3 CTAs per SM */
+template <typename T, bool BIG>
+__global__ void __launch_bounds__(BIG ? 512 : 256, (!BIG && sizeof(T) == 4) ? 3 : 1) k_rows(const __grid_constant__ Program P, const RowArgs<T> A) {
   typedef typename cplx_of<T>::type C;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   C *sm = reinterpret_cast<C *>(smem_raw);

@@ -99,6 +99,9 @@ struct Geo {
    * both spread over the banks.  npad = geo_pad(n-1) + 1 rows are allocated. */
   int32_t sh[3];
   int32_t npad;
+  /* digit fields of the reversal: digit q of frequency f sits at bits [fs[q], fs[q]+lg[q]) and moves to slot bits
+   * starting at ps[q]; fm[q] is its mask (0 for unused passes) */
+  int32_t fs[4], ps[4], fm[4];
 };
 
 #endif
