@@ -303,7 +303,7 @@ int build_program(pss_system *s) {
     auto radial = [](const DOp &d) { return d.p == 0 && d.a[0] == 0 && d.a[1] == 0 && d.a[2] == 0 && d.zflags == 0 && d.m <= 4; };
     bool ok = env_int("PSS_RADIAL", 1) != 0 && P.ndyn == 1 && P.ngrp <= 1 && P.nfac <= 1 &&
               P.dyn[0].lin_beg == P.dyn[0].lin_end;
-    if (ok && P.dyn[0].noisy && (P.dyn[0].noise_qpow < 0 || (P.dyn[0].noise_qpow & 1))) ok = false;
+    if (ok && P.dyn[0].noisy && (P.dyn[0].noise_qpow < 0 || (P.dyn[0].noise_qpow & 1) || P.dyn[0].noise_qpow > 14)) ok = false;
     for (int e = P.dyn[0].lhs_beg; ok && e < P.dyn[0].lhs_end; ++e) ok = radial(P.lin[e]);
     if (ok && P.ngrp == 1) ok = radial(P.grp[0].outer);
     if (ok && P.nfac == 1)

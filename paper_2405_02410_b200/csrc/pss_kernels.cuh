@@ -122,8 +122,11 @@ __global__ void __launch_bounds__(256, sizeof(T) == 4 ? 3 : 2) k_update(const __
           }
           const DDyn &d = P.dyn[0];
           if (d.noisy) {
+            const T q4 = mq.q2 * mq.q2; /* (q^2)^nhp, nhp <= 4, branch-free */
             T qa = (T)d.noise_c;
-            for (int i = 0; i < P.rad_nhp; ++i) qa *= mq.q2;
+            qa *= (P.rad_nhp & 1) ? mq.q2 : (T)1;
+            qa *= (P.rad_nhp & 2) ? q4 : (T)1;
+            qa *= (P.rad_nhp & 4) ? q4 * q4 : (T)1;
             const T amp = sqrt(qa);
             const C z = noise_z<T>(P, d.field_id, A.step, lq.k0, P.ndim == 3 ? lq.k1 : k, P.ndim == 3 ? k : 0);
             num.x += amp * z.x;

@@ -211,7 +211,10 @@ __device__ __forceinline__ typename cplx_of<T>::type noise_z(const Program &P, i
 template <>
 __device__ __forceinline__ float2 noise_z<float>(const Program &P, int field, unsigned long long step, int k0, int k1, int k2) {
   const long long n1 = P.n[1], n2 = P.n[2], nxh = P.nxh;
-  long long m = ((long long)k2 * n1 + k1) * nxh + k0;
+  /* 32-bit index arithmetic whenever the half-spectrum has fewer than 2^31 modes */
+  const bool small = (long long)P.nxh * P.n[1] * P.n[2] < 0x7fffffffLL;
+  long long m = small ? (long long)(unsigned)(((unsigned)k2 * (unsigned)P.n[1] + (unsigned)k1) * (unsigned)P.nxh + (unsigned)k0)
+                      : ((long long)k2 * n1 + k1) * nxh + k0;
   NoiseKey K;
   K.k0 = P.seed_lo;
   K.k1 = P.seed_hi;
