@@ -292,6 +292,17 @@ def main():
                               "frac_model": b_model / (step_ms * 1e-3) / 1e9 / peak,
                               "frac_alg_of_8TBs": b_alg / (step_ms * 1e-3) / 1e9 / 8000.0},
         }
+        # secondary reading: the kernels are issue-bound, so also report the issue-slot fraction of the dominant kernel
+        # (ncu smsp__inst_executed.sum of the committed capture / its step count, against 4 schedulers x SMs x clock)
+        tr = line["roofline"]["traffic"]
+        if tr:
+            nsm = torch.cuda.get_device_properties(dev).multi_processor_count
+            mhz = (clocks or {}).get("sm_mhz") or 1965.0
+            wi_step = tr["warp_instr_per_launch"] / tr["timesteps_per_launch"]
+            t_dom = dom_ms * 1e-3 / (prof_n if dom == "k_fused2d" else 1)
+            line["roofline"]["issue"] = {"bound": "alu", "unit": "warp-instr/s", "achieved": wi_step / t_dom,
+                                         "peak": 4.0 * nsm * mhz * 1e6, "frac": wi_step / t_dom / (4.0 * nsm * mhz * 1e6),
+                                         "note": "instruction-issue slots: 4 schedulers per SM x 1 warp-instr per clock"}
         if not args.no_cpu_baseline and world == 1:
             r, n, el, cores = oracle_rate(cfg, args.prec, args.cpu_budget, 64)
             line["cpu_baseline"] = {"value": r, "unit": "timesteps/s", "cores": cores, "kind": "oracle",
@@ -353,9 +364,10 @@ def ncu_traffic(workload, kernel):
     try:
         with open(p) as f:
             for ln in f.read().splitlines()[1:]:
-                w, k, b, n, src = ln.split(",")
+                w, k, b, n, wi, src = ln.split(",")
                 if w == workload and k == kernel:
-                    return {"dram_bytes_per_launch": int(b), "timesteps_per_launch": int(n), "source": src}
+                    return {"dram_bytes_per_launch": int(b), "timesteps_per_launch": int(n),
+                            "warp_instr_per_launch": int(wi), "source": src}
     except Exception:
         pass
     return None
