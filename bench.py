@@ -149,6 +149,8 @@ def main():
     ap.add_argument("--impl", default="pss", choices=["pss", "reference"])
     ap.add_argument("--ref-budget", type=float, default=20.0, help="seconds of oracle work for the reference arm")
     ap.add_argument("--cpu-budget", type=float, default=12.0, help="seconds of oracle work for cpu_baseline")
+    ap.add_argument("--replicas", type=int, default=1,
+                    help="ensemble: R independent realisations stepped in the same launches (value counts replica-steps)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-compare", action="store_true", help="skip the cuFFT+cuRAND comparison step (2D Model B only)")
     args = ap.parse_args()
@@ -174,7 +176,9 @@ def main():
 
     # replicas only: every rank advances its own realisation (seed + rank), no data-path collective
     cfg_r = replicas.rank_config(cfg, rank)
-    g, ids = wl.build(pss, cfg_r, prec=args.prec, device="cuda:%d" % local_rank)
+    R = max(1, args.replicas)
+    cfg_r["seed"] = cfg["seed"] + rank * R          # replica r of rank k is the realisation seed + k*R + r
+    g, ids = wl.build(pss, cfg_r, prec=args.prec, device="cuda:%d" % local_rank, set_ic=False, replicas=R)
     dyn_names = list(cfg["ic"].keys())
     sites = int(np.prod(cfg["n"]))
     rsize = 4 if args.prec == "f32" else 8
@@ -186,9 +190,15 @@ def main():
             dist.barrier()
         torch.cuda.synchronize(dev)
 
+    ics = [wl.initial_conditions(dict(cfg_r, seed=cfg_r["seed"] + r), g.rdtype) for r in range(R)]
+
     def reset_state():
-        for name, arr in wl.initial_conditions(cfg_r, g.rdtype).items():
-            g.set_field(ids[name], arr)
+        for r in range(R):
+            g.select_replica(r)
+            for name, arr in ics[r].items():
+                g.set_field(ids[name], arr)
+
+    reset_state()
 
     # nematic (A20): the literal parameters blow up after ~400 steps -> re-seed before every bench step
     reseed = cfg["model"] == "nematic"
@@ -220,16 +230,20 @@ def main():
     clocks = sampler.stop() if sampler else None
 
     # ---- e2e: host buffers through the public API, copies inside the timed region ----
-    host_in = {name: torch.from_numpy(arr).pin_memory() for name, arr in wl.initial_conditions(cfg_r, g.rdtype).items()}
-    host_out = {name: torch.empty_like(t).pin_memory() for name, t in host_in.items()}
+    host_in = [{name: torch.from_numpy(arr).pin_memory() for name, arr in ics[r].items()} for r in range(R)]
+    host_out = [{name: torch.empty_like(t).pin_memory() for name, t in host_in[r].items()} for r in range(R)]
     e2e_steps = max(2, min(args.steps, 5))
 
     def e2e_once():
-        for name in dyn_names:
-            g.set_field(ids[name], host_in[name].numpy())
+        for r in range(R):
+            g.select_replica(r)
+            for name in dyn_names:
+                g.set_field(ids[name], host_in[r][name].numpy())
         g.step(inner)
-        for name in dyn_names:
-            g.get_field(ids[name], out=host_out[name].numpy())
+        for r in range(R):
+            g.select_replica(r)
+            for name in dyn_names:
+                g.get_field(ids[name], out=host_out[r][name].numpy())
 
     e2e_once()
     barrier()
@@ -238,7 +252,7 @@ def main():
         e2e_once()
     torch.cuda.synchronize(dev)
     e2e_s = time.perf_counter() - t0
-    finite = all(bool(np.isfinite(host_out[n].numpy()).all()) for n in dyn_names)
+    finite = all(bool(np.isfinite(host_out[r][n].numpy()).all()) for r in range(R) for n in dyn_names)
 
     # ---- per-kernel device times (CUDA events around every launch) for the roofline of the dominant kernel ----
     if reseed:
@@ -248,37 +262,38 @@ def main():
     barrier()
 
     # max over ranks of the timed totals; sum of units
-    (total_ms, e2e_s), steps_all = replicas.reduce_timings([total_ms, e2e_s], args.steps * inner, device=dev)
+    (total_ms, e2e_s), steps_all = replicas.reduce_timings([total_ms, e2e_s], args.steps * inner * R, device=dev)
     value = steps_all / (total_ms * 1e-3)
-    e2e_value = world * e2e_steps * inner / e2e_s
+    e2e_value = world * e2e_steps * inner * R / e2e_s
 
     if rank == 0:
         peak, peak_src = measured_peak()
         S = sites * rsize
         b_alg = g.model_bytes_per_step(True)
         b_model = g.model_bytes_per_step(False)
-        step_ms = total_ms / (args.steps * inner)
+        step_ms = total_ms / (args.steps * inner)   # one launch sequence advances all R replicas by one time step
         # dominant kernel by share of device time
         shares = {k: v[0] * v[1] for k, v in prof.items() if v[1] > 0}
         dom = max(shares, key=shares.get)
         dom_ms = prof[dom][0]
         P = g  # algorithmic bytes per launch of each kernel family
-        kb = kernel_bytes(cfg, S, g, prof_n)
+        kb = kernel_bytes(cfg, S * R, g, prof_n)
         ach = kb[dom] / (dom_ms * 1e-3) / 1e9
         line = {
             "metric": "timesteps/s", "value": value, "unit": "timesteps/s", "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": args.prec, "data": "synthetic",
-            "site_updates_per_s": value * sites, "us_per_timestep": step_ms * 1e3,
+            "site_updates_per_s": value * sites, "us_per_timestep": step_ms * 1e3, "us_per_replica_timestep": step_ms * 1e3 / R,
             "config": {"workload": args.workload, "lattice": list(cfg["n"]), "precision": args.prec,
-                       "timesteps_per_bench_step": inner, "parallelism": "replicas only (one realisation per GPU)",
+                       "timesteps_per_bench_step": inner, "replicas_per_gpu": R,
+                       "parallelism": "replicas only (independent realisations; value counts replica time steps)",
                        "l2": "flushed between timed bench steps (256 MiB written); inside a bench step the "
                              "time stepper reuses its own state, as the workload does",
                        "final_state_finite": finite},
             "gpu_launches": int(launches_timed),
             "clocks": clocks,
             "e2e": {"value": e2e_value, "unit": "timesteps/s",
-                    "h2d_bytes_per_step": len(dyn_names) * S, "d2h_bytes_per_step": len(dyn_names) * S,
+                    "h2d_bytes_per_step": len(dyn_names) * S * R, "d2h_bytes_per_step": len(dyn_names) * S * R,
                     "note": "pss_set_field(host) + pss_step(%d) + pss_get_field(host) per bench step" % inner},
             "roofline": {"bound": "hbm", "kernel": dom, "achieved": ach, "peak": peak, "unit": "GB/s",
                          "frac": ach / peak, "traffic": ncu_traffic(args.workload, dom), "peak_source": peak_src,

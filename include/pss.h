@@ -81,6 +81,14 @@ int pss_add_term(pss_system *, int field, const pss_op *outer, int nfactors, con
 int pss_set_noise(pss_system *, int field, double D, int q_power);
 /* de-aliasing rule: PAPER = cutoff 2/(n+1) per factor field, n its highest order. */
 int pss_set_dealias(pss_system *, int rule);
+/* Ensemble (stochastic studies need many realisations): the system holds
+ * `nreplicas` independent realisations of the same field system and pss_step advances all of them in the same
+ * launches (grid dimension y).  Replica r is, bit for bit, the system created with seed + r.  Call before
+ * pss_finalize; 1 <= nreplicas <= 65535.  The persistent 1024^2 kernel is used for nreplicas == 1 only. */
+int pss_set_replicas(pss_system *, int nreplicas);
+/* which replica pss_set_field / pss_get_field / pss_get_field_fourier / pss_debug_noise address (default 0) */
+int pss_select_replica(pss_system *, int replica);
+int pss_replicas(const pss_system *);
 /* validate, freeze the term list, plan the kernels; *workspace_bytes = device bytes pss_bind needs. */
 int pss_finalize(pss_system *, size_t *workspace_bytes);
 /* device_workspace: DEVICE pointer, 256-byte aligned, >= workspace_bytes, zero-initialised by this

@@ -19,7 +19,7 @@ DEALIAS_PAPER, DEALIAS_TWO_THIRDS, DEALIAS_OFF = 0, 1, 2
 OK, EINVAL, EUNSUPPORTED, ESTATE, ECUDA = 0, -1, -2, -3, -4
 
 SYMBOLS = ["pss_create", "pss_add_field", "pss_add_linear", "pss_add_aux_def", "pss_add_term",
-           "pss_set_noise", "pss_set_dealias", "pss_finalize", "pss_bind", "pss_set_field", "pss_step",
+           "pss_set_noise", "pss_set_dealias", "pss_set_replicas", "pss_select_replica", "pss_replicas", "pss_finalize", "pss_bind", "pss_set_field", "pss_step",
            "pss_get_field", "pss_get_field_fourier", "pss_debug_noise", "pss_profile_step", "pss_uses_fused_kernel", "pss_launch_count",
            "pss_model_bytes_per_step", "pss_step_count", "pss_strerror", "pss_last_cuda_error",
            "pss_destroy"]
@@ -60,6 +60,9 @@ def lib():
         L.pss_add_term.argtypes = [P, C.c_int, C.POINTER(_Op), C.c_int, C.POINTER(C.c_int)]
         L.pss_set_noise.argtypes = [P, C.c_int, C.c_double, C.c_int]
         L.pss_set_dealias.argtypes = [P, C.c_int]
+        L.pss_set_replicas.argtypes = [P, C.c_int]
+        L.pss_select_replica.argtypes = [P, C.c_int]
+        L.pss_replicas.argtypes = [P]
         L.pss_finalize.argtypes = [P, C.POINTER(C.c_size_t)]
         L.pss_bind.argtypes = [P, P, C.c_size_t, P]
         L.pss_set_field.argtypes = [P, C.c_int, P, C.c_int]
@@ -100,7 +103,7 @@ def _n3(n):
 class System:
     """One field system on the GPU.  ``n`` and ``dx`` are given x first: (Nx[, Ny[, Nz]])."""
 
-    def __init__(self, n, dx, dt, prec="f32", seed=0, device="cuda:0", stream=None):
+    def __init__(self, n, dx, dt, prec="f32", seed=0, device="cuda:0", stream=None, replicas=1):
         self.n = tuple(int(v) for v in n)
         self.ndim = len(self.n)
         self.prec = {"f32": F32, "f64": F64, F32: F32, F64: F64}[prec]
@@ -116,6 +119,8 @@ class System:
                               C.c_uint64(int(seed)))
         if rc != 0:
             raise PssError(rc)
+        if int(replicas) != 1:
+            self.set_replicas(replicas)
         self.shape = self.n[::-1]
         self.hshape = self.n[::-1][:-1] + (self.n[0] // 2 + 1,)
 
@@ -151,6 +156,17 @@ class System:
 
     def set_noise(self, field, D, q_power):
         self._chk(lib().pss_set_noise(self._h, int(field), float(D), int(q_power)))
+
+    def set_replicas(self, nreplicas):
+        """ensemble of independent realisations (replica r = seed + r), stepped together; before finalize"""
+        self._chk(lib().pss_set_replicas(self._h, int(nreplicas)))
+
+    def select_replica(self, r):
+        self._chk(lib().pss_select_replica(self._h, int(r)))
+
+    @property
+    def replicas(self):
+        return int(lib().pss_replicas(self._h))
 
     def set_dealias(self, rule):
         self._chk(lib().pss_set_dealias(self._h, int(rule)))

@@ -53,6 +53,7 @@ struct pss_system {
   int prec;
   uint64_t seed;
   int dealias;
+  int nrep, sel; /* ensemble: replicas of the same field system (replica r = seed + r), selected replica for set/get */
   bool finalized, bound, psix_valid;
   uint64_t step;
   std::vector<FieldH> fields;
@@ -365,7 +366,7 @@ bool real_op(const DOp &d) { return ((d.a[0] + d.a[1] + d.a[2]) & 1) == 0; }
 bool fused2d_eligible(const pss_system *s) {
   const Program &P = s->P;
   if (env_int("PSS_FUSED", 1) == 0) return false;
-  if (s->ndim != 2 || s->prec != PSS_F32 || s->n[0] != f2d::N || s->n[1] != f2d::N) return false;
+  if (s->ndim != 2 || s->prec != PSS_F32 || s->n[0] != f2d::N || s->n[1] != f2d::N || s->nrep != 1) return false;
   if (P.ndyn != 1 || P.nfac != 1 || P.ngrp != 1) return false;
   if (P.dyn[0].lin_beg != P.dyn[0].lin_end) return false;
   if (!real_op(P.grp[0].outer)) return false;
@@ -474,9 +475,10 @@ void carve_workspace(pss_system *s) {
   const Program &P = s->P;
   size_t off = 0;
   const size_t arr = align_up((size_t)s->M * s->csize, 256);
-  s->off_state = off; off += arr * (size_t)P.ndyn;
-  s->off_psix = off;  off += arr * (size_t)(P.nfac > 0 ? P.nfac : 0);
-  s->off_phat = off;  off += arr * (size_t)(P.ngrp > 0 ? P.ngrp : 0);
+  const size_t R = (size_t)s->nrep; /* arrays of one kind: [replica][field][M] */
+  s->off_state = off; off += arr * (size_t)P.ndyn * R;
+  s->off_psix = off;  off += arr * (size_t)(P.nfac > 0 ? P.nfac : 0) * R;
+  s->off_phat = off;  off += arr * (size_t)(P.ngrp > 0 ? P.ngrp : 0) * R;
   s->off_scratch = off; off += arr;
   s->off_ureal = off; off += align_up((size_t)s->N * s->rsize, 256);
   for (int j = 0; j < 3; ++j) { s->off_tw[j] = off; off += align_up((size_t)s->n[j] * s->csize, 256); }
@@ -555,7 +557,7 @@ void prof_mark(pss_system *s, int kind, bool begin) {
   if (begin) s->prof_kind.push_back(kind);
 }
 
-template <typename T> int launch_mid(pss_system *s, int sgn, size_t off, int nbatch, int kx_count, bool factor_mask = false) {
+template <typename T> int launch_mid(pss_system *s, int sgn, size_t off, int nbatch, int kx_count, bool factor_mask = false, int nrep = 1) {
   MidArgs<T> a;
   std::memset(&a, 0, sizeof(a));
   a.nx = (int)s->n[0];
@@ -568,8 +570,9 @@ template <typename T> int launch_mid(pss_system *s, int sgn, size_t off, int nba
   a.nz = (int)s->n[2];
   a.W = s->plan.mid_W;
   a.kx_count = kx_count;
+  a.nbatch = nbatch;
   a.geo = s->plan.geo[1];
-  dim3 grid((unsigned)(s->n[2] / s->plan.mid_W), (unsigned)kx_count, (unsigned)nbatch);
+  dim3 grid((unsigned)(s->n[2] / s->plan.mid_W), (unsigned)kx_count, (unsigned)(nbatch * nrep));
   prof_mark(s, KIND_MID, true);
   if (sgn < 0) k_mid<-1, T><<<grid, s->plan.mid_threads, s->plan.mid_smem, s->stream>>>(a);
   else k_mid<+1, T><<<grid, s->plan.mid_threads, s->plan.mid_smem, s->stream>>>(a);
@@ -596,11 +599,12 @@ template <typename T> int launch_update(pss_system *s, int prologue, uint64_t st
   a.step = step;
   a.geo = s->plan.geo[s->ndim - 1];
   prof_mark(s, KIND_UPDATE, true);
-  if (P.rad_ok) k_update<T, true><<<s->plan.upd_blocks, s->plan.upd_threads, s->plan.upd_smem, s->stream>>>(P, a);
-  else k_update<T, false><<<s->plan.upd_blocks, s->plan.upd_threads, s->plan.upd_smem, s->stream>>>(P, a);
+  const dim3 grid((unsigned)s->plan.upd_blocks, (unsigned)s->nrep);
+  if (P.rad_ok) k_update<T, true><<<grid, s->plan.upd_threads, s->plan.upd_smem, s->stream>>>(P, a);
+  else k_update<T, false><<<grid, s->plan.upd_threads, s->plan.upd_smem, s->stream>>>(P, a);
   prof_mark(s, KIND_UPDATE, false);
   CKL("k_update");
-  if (s->ndim == 3 && P.nfac > 0) return launch_mid<T>(s, +1, s->off_psix, P.nfac, s->plan.kx_keep_max, true);
+  if (s->ndim == 3 && P.nfac > 0) return launch_mid<T>(s, +1, s->off_psix, P.nfac, s->plan.kx_keep_max, true, s->nrep);
   return PSS_OK;
 }
 
@@ -616,11 +620,12 @@ template <typename T> int launch_rows(pss_system *s) {
   a.Wc = s->plan.row_Wc;
   a.geo = s->plan.geo[0];
   prof_mark(s, KIND_ROWS, true);
-  if (s->plan.row_threads > 256) k_rows<T, true><<<s->plan.row_blocks, s->plan.row_threads, s->plan.row_smem, s->stream>>>(P, a);
-  else k_rows<T, false><<<s->plan.row_blocks, s->plan.row_threads, s->plan.row_smem, s->stream>>>(P, a);
+  const dim3 grid((unsigned)s->plan.row_blocks, (unsigned)s->nrep);
+  if (s->plan.row_threads > 256) k_rows<T, true><<<grid, s->plan.row_threads, s->plan.row_smem, s->stream>>>(P, a);
+  else k_rows<T, false><<<grid, s->plan.row_threads, s->plan.row_smem, s->stream>>>(P, a);
   prof_mark(s, KIND_ROWS, false);
   CKL("k_rows");
-  if (s->ndim == 3) return launch_mid<T>(s, -1, s->off_phat, P.ngrp, P.nxh);
+  if (s->ndim == 3) return launch_mid<T>(s, -1, s->off_phat, P.ngrp, P.nxh, false, s->nrep);
   return PSS_OK;
 }
 
@@ -661,7 +666,7 @@ template <typename T> int do_steps(pss_system *s, int64_t nsteps) {
     a.nsteps = nsteps;
     a.step0 = s->step;
     a.geo = s->plan.geo[0];
-    k_step1d<T><<<1, s->plan.one_threads, s->plan.one_smem, s->stream>>>(P, a);
+    k_step1d<T><<<s->nrep, s->plan.one_threads, s->plan.one_smem, s->stream>>>(P, a);
     CKL("k_step1d");
     s->step += (uint64_t)nsteps;
     return PSS_OK;
@@ -688,7 +693,8 @@ template <typename T> int do_set_field(pss_system *s, int slot, const void *src,
   }
   UserArgs<T> a;
   a.real = const_cast<T *>(real);
-  a.arr = carr<T>(s, s->off_state, slot);
+  const int sidx = s->sel * s->P.ndyn + slot; /* state array of the selected replica */
+  a.arr = carr<T>(s, s->off_state, sidx);
   a.tw = twp<T>(s, 0);
   a.nx = (int)s->n[0];
   a.ny = (int)s->n[1];
@@ -701,12 +707,12 @@ template <typename T> int do_set_field(pss_system *s, int slot, const void *src,
   k_user_x<-1, T><<<blocks, round_threads(s->n[0] / 4), (size_t)s->plan.geo[0].npad * sizeof(typename cplx_of<T>::type), s->stream>>>(a);
   CKL("k_user_x");
   if (s->ndim == 3) {
-    const int rc = launch_mid<T>(s, -1, s->off_state + (size_t)slot * (size_t)arr_stride(s) * s->csize, 1, s->P.nxh);
+    const int rc = launch_mid<T>(s, -1, s->off_state + (size_t)sidx * (size_t)arr_stride(s) * s->csize, 1, s->P.nxh);
     if (rc != PSS_OK) return rc;
   }
   if (s->ndim >= 2) {
     LastArgs<T> l;
-    l.arr = carr<T>(s, s->off_state, slot);
+    l.arr = carr<T>(s, s->off_state, sidx);
     l.tw = twp<T>(s, s->ndim - 1);
     l.n = (int)s->n[s->ndim - 1];
     l.nlines = (int)(s->M / l.n);
@@ -721,7 +727,7 @@ template <typename T> int do_set_field(pss_system *s, int slot, const void *src,
 
 template <typename T> int do_get_field(pss_system *s, int slot, void *dst, int on_device) {
   typedef typename cplx_of<T>::type C;
-  CK(cudaMemcpyAsync(s->ws + s->off_scratch, carr<T>(s, s->off_state, slot), (size_t)s->M * sizeof(C),
+  CK(cudaMemcpyAsync(s->ws + s->off_scratch, carr<T>(s, s->off_state, s->sel * s->P.ndyn + slot), (size_t)s->M * sizeof(C),
                      cudaMemcpyDeviceToDevice, s->stream));
   if (s->ndim >= 2) {
     LastArgs<T> l;
@@ -761,7 +767,7 @@ template <typename T> int do_get_field(pss_system *s, int slot, void *dst, int o
 template <typename T> int do_get_fourier(pss_system *s, int slot, void *dst, int on_device) {
   typedef typename cplx_of<T>::type C;
   C *out = on_device ? (C *)dst : carr<T>(s, s->off_scratch, 0);
-  k_to_logical<T><<<592, 256, 0, s->stream>>>(carr<T>(s, s->off_state, slot), out, s->P.nxh, (int)s->n[1], (int)s->n[2]);
+  k_to_logical<T><<<592, 256, 0, s->stream>>>(carr<T>(s, s->off_state, s->sel * s->P.ndyn + slot), out, s->P.nxh, (int)s->n[1], (int)s->n[2]);
   CKL("k_to_logical");
   if (!on_device) {
     CK(cudaMemcpyAsync(dst, out, (size_t)s->M * sizeof(C), cudaMemcpyDeviceToHost, s->stream));
@@ -776,7 +782,7 @@ template <typename T> int do_debug_noise(pss_system *s, int field, uint64_t step
   C *dz = nullptr;
   if (bits) CK(cudaMalloc(&dbits, (size_t)s->M * 4 * sizeof(uint32_t)));
   if (z) CK(cudaMalloc(&dz, (size_t)s->M * sizeof(C)));
-  k_debug_noise<T><<<592, 256, 0, s->stream>>>(s->P, field, step, dbits, dz);
+  k_debug_noise<T><<<592, 256, 0, s->stream>>>(s->P, (unsigned)s->sel, field, step, dbits, dz);
   CKL("k_debug_noise");
   if (bits) CK(cudaMemcpyAsync(bits, dbits, (size_t)s->M * 4 * sizeof(uint32_t), cudaMemcpyDeviceToHost, s->stream));
   if (z) CK(cudaMemcpyAsync(z, dz, (size_t)s->M * sizeof(C), cudaMemcpyDeviceToHost, s->stream));
@@ -810,6 +816,8 @@ int pss_create(pss_system **out, int ndim, const int64_t n[3], const double dx[3
   s->prec = (int)prec;
   s->seed = seed;
   s->dealias = PSS_DEALIAS_PAPER;
+  s->nrep = 1;
+  s->sel = 0;
   s->finalized = s->bound = s->psix_valid = false;
   s->step = 0;
   s->csize = prec == PSS_F32 ? 8 : 16;
@@ -891,6 +899,24 @@ int pss_set_dealias(pss_system *s, int rule) {
   s->dealias = rule;
   return PSS_OK;
 }
+
+int pss_set_replicas(pss_system *s, int nreplicas) {
+  if (!s) return PSS_EINVAL;
+  if (s->finalized) return PSS_ESTATE;
+  if (nreplicas < 1) return PSS_EINVAL;
+  if (nreplicas > 65535) return PSS_EUNSUPPORTED;
+  s->nrep = nreplicas;
+  s->sel = 0;
+  return PSS_OK;
+}
+
+int pss_select_replica(pss_system *s, int replica) {
+  if (!s || replica < 0 || replica >= s->nrep) return PSS_EINVAL;
+  s->sel = replica;
+  return PSS_OK;
+}
+
+int pss_replicas(const pss_system *s) { return s ? s->nrep : 0; }
 
 int pss_finalize(pss_system *s, size_t *workspace_bytes) {
   if (!s) return PSS_EINVAL;
@@ -1022,7 +1048,7 @@ int pss_uses_fused_kernel(const pss_system *s) { return (s && s->finalized && s-
 double pss_model_bytes_per_step(const pss_system *s, int pruned) {
   if (!s || !s->finalized) return 0.0;
   const Program &P = s->P;
-  const double S = (double)s->N * (double)s->rsize;
+  const double S = (double)s->N * (double)s->rsize * (double)s->nrep;
   if (s->ndim == 1) return 2.0 * P.ndyn * S;
   double c1 = 0.0, c2 = 0.0; /* sum over factors of the kept fraction per axis, and its square */
   for (int f = 0; f < P.nfac; ++f) {

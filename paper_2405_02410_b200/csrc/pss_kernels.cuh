@@ -77,6 +77,10 @@ __global__ void __launch_bounds__(256, sizeof(T) == 4 ? 3 : 2) k_update(const __
   C *sm = reinterpret_cast<C *>(smem_raw);
   const int n = A.n, W = A.W, lgn = A.lgn, lgW = A.lgW;
   const int line0 = blockIdx.x * W;
+  const unsigned rep = blockIdx.y; /* ensemble replica: arrays [replica][field][M] */
+  C *const st_base = A.state + (size_t)rep * P.ndyn * A.M;
+  C *const psix_base = A.psix + (size_t)rep * P.nfac * A.M;
+  const C *const phat_base = A.phat + (size_t)rep * P.ngrp * A.M;
   const int nl = min(W, A.nlines - line0);
   const int nb0 = max(P.ngrp, P.ndyn);
   const int RS = (nb0 + (P.nfac > 1 ? 1 : 0)) * W; /* columns per smem row */
@@ -91,7 +95,7 @@ __global__ void __launch_bounds__(256, sizeof(T) == 4 ? 3 : 2) k_update(const __
   /* ---- phase A: forward FFT of the groups along the last axis ---- */
   if (!A.prologue && P.ngrp > 0) {
     for (int g = 0; g < P.ngrp; ++g) {
-      const C *src = A.phat + (size_t)g * A.M + (size_t)line0 * n;
+      const C *src = phat_base + (size_t)g * A.M + (size_t)line0 * n;
 #pragma unroll 4
       for (int idx = tid; idx < (W << lgn); idx += nt) {
         const int c = idx >> lgn, j = idx & (n - 1);
@@ -110,7 +114,7 @@ __global__ void __launch_bounds__(256, sizeof(T) == 4 ? 3 : 2) k_update(const __
       C *srow = sm + (size_t)geo_pad(A.geo, geo_slot_fast(A.geo, k)) * RS + c;
       const size_t gi = (size_t)line * n + k;
       if (RAD) {
-        const C phi = A.state[gi];
+        const C phi = st_base[gi];
         if (!A.prologue) {
           const ModeQ<T> mq = line_mode<T>(P, lq, k, n, qs_last);
           C num = phi;
@@ -128,13 +132,13 @@ __global__ void __launch_bounds__(256, sizeof(T) == 4 ? 3 : 2) k_update(const __
             qa *= (P.rad_nhp & 2) ? q4 : (T)1;
             qa *= (P.rad_nhp & 4) ? q4 * q4 : (T)1;
             const T amp = sqrt(qa);
-            const C z = noise_z<T>(P, d.field_id, A.step, lq.k0, P.ndim == 3 ? lq.k1 : k, P.ndim == 3 ? k : 0);
+            const C z = noise_z<T>(P, rep, d.field_id, A.step, lq.k0, P.ndim == 3 ? lq.k1 : k, P.ndim == 3 ? k : 0);
             num.x += amp * z.x;
             num.y += amp * z.y;
           }
           const T inv = (T)1 / ((T)1 - dt * horner4<T>(radL, mq.q2));
           const C out = mk<C, T>(num.x * inv, num.y * inv);
-          A.state[gi] = out;
+          st_base[gi] = out;
           srow[0] = out;
         } else {
           srow[0] = phi;
@@ -142,7 +146,7 @@ __global__ void __launch_bounds__(256, sizeof(T) == 4 ? 3 : 2) k_update(const __
       } else {
       C phi[PSS_P_MAX_DYN];
 #pragma unroll
-      for (int i = 0; i < PSS_P_MAX_DYN; ++i) phi[i] = (i < P.ndyn) ? A.state[(size_t)i * A.M + gi] : zero;
+      for (int i = 0; i < PSS_P_MAX_DYN; ++i) phi[i] = (i < P.ndyn) ? st_base[(size_t)i * A.M + gi] : zero;
       if (!A.prologue) {
         const ModeQ<T> mq = line_mode<T>(P, lq, k, n, qs_last);
         C out[PSS_P_MAX_DYN];
@@ -159,7 +163,7 @@ __global__ void __launch_bounds__(256, sizeof(T) == 4 ? 3 : 2) k_update(const __
             C num = mk<C, T>(phi[i].x + dt * N.x, phi[i].y + dt * N.y);
             if (d.noisy) {
               const T amp = noise_amp<T>(d, mq);
-              const C z = noise_z<T>(P, d.field_id, A.step, lq.k0, P.ndim == 3 ? lq.k1 : k, P.ndim == 3 ? k : 0);
+              const C z = noise_z<T>(P, rep, d.field_id, A.step, lq.k0, P.ndim == 3 ? lq.k1 : k, P.ndim == 3 ? k : 0);
               num.x += amp * z.x;
               num.y += amp * z.y;
             }
@@ -174,7 +178,7 @@ __global__ void __launch_bounds__(256, sizeof(T) == 4 ? 3 : 2) k_update(const __
 #pragma unroll
         for (int i = 0; i < PSS_P_MAX_DYN; ++i)
           if (i < P.ndyn) {
-            A.state[(size_t)i * A.M + gi] = out[i];
+            st_base[(size_t)i * A.M + gi] = out[i];
             srow[i * W] = out[i];
           }
       } else {
@@ -231,7 +235,7 @@ __global__ void __launch_bounds__(256, sizeof(T) == 4 ? 3 : 2) k_update(const __
     }
     __syncthreads();
     fft_dit<+1, T>(A.geo, sm + wb * W, A.tw, W, RS);
-    C *dst = A.psix + (size_t)f * A.M + (size_t)line0 * n;
+    C *dst = psix_base + (size_t)f * A.M + (size_t)line0 * n;
 #pragma unroll 4
     for (int idx = tid; idx < (W << lgn); idx += nt) {
       const int c = idx >> lgn, j = idx & (n - 1);
@@ -262,6 +266,8 @@ __global__ void __launch_bounds__(BIG ? 512 : 256, (!BIG && sizeof(T) == 4) ? 3 
   const int nx = A.nx, nxh = nx / 2 + 1, Wc = A.Wc, lgWc = 31 - __clz(Wc); /* Wc is a power of two */
   const int RS = (P.nfac + (P.ngrp > 1 ? 1 : 0)) * Wc;
   const long long r0 = (long long)blockIdx.x * (2 * Wc);
+  const C *const psix_base = A.psix + (size_t)blockIdx.y * P.nfac * A.M; /* ensemble replica blockIdx.y */
+  C *const phat_base = A.phat + (size_t)blockIdx.y * P.ngrp * A.M;
   const int tid = threadIdx.x, nt = blockDim.x;
   const C zero = mk<C, T>((T)0, (T)0);
 
@@ -275,7 +281,7 @@ __global__ void __launch_bounds__(BIG ? 512 : 256, (!BIG && sizeof(T) == 4) ? 3 
       cut = (nx + nn - 1) / nn; /* kx kept iff nn*kx < nx */
       if (cut > nxh) cut = nxh;
     }
-    const C *src = A.psix + (size_t)f * A.M + r0;
+    const C *src = psix_base + (size_t)f * A.M + r0;
     for (int idx = tid; idx < cut * Wc; idx += nt) {
       const int c = idx & (Wc - 1), kx = idx >> lgWc;
       const C *p = src + (size_t)kx * A.R + 2 * c;
@@ -325,7 +331,7 @@ __global__ void __launch_bounds__(BIG ? 512 : 256, (!BIG && sizeof(T) == 4) ? 3 
     }
     __syncthreads();
     fft_dit<-1, T>(A.geo, sm + wb * Wc, A.tw, Wc, RS);
-    C *dst = A.phat + (size_t)g * A.M + r0;
+    C *dst = phat_base + (size_t)g * A.M + r0;
     for (int idx = tid; idx < nxh * Wc; idx += nt) {
       const int c = idx & (Wc - 1), kx = idx >> lgWc;
       const C z = sm[(size_t)geo_pad(A.geo, kx) * RS + wb * Wc + c];
@@ -347,6 +353,7 @@ template <typename T> struct MidArgs {
   long long M;
   int ny, nz, W;
   int kx_count; /* lines with kx >= kx_count are skipped (de-aliased away) */
+  int nbatch;   /* arrays per replica */
   int nx;
   int nn[PSS_P_MAX_FAC]; /* per batch entry: order+1 of the de-aliasing rule, 0 = no mask.  Rows ky and lines
                             kx outside the kept band were never written by k_update: read them as zero */
@@ -360,7 +367,7 @@ template <int SGN, typename T> __global__ void __launch_bounds__(256) k_mid(cons
   const int W = A.W, ny = A.ny;
   const int kx = blockIdx.y;
   if (kx >= A.kx_count) return;
-  const int nn = A.nn[blockIdx.z];
+  const int nn = A.nn[blockIdx.z % A.nbatch]; /* blockIdx.z runs over [replica][array] */
   if (nn && nn * kx >= A.nx) return;
   C *base = A.arr + (size_t)blockIdx.z * A.M + (size_t)kx * ny * A.nz + (size_t)blockIdx.x * W;
   for (int idx = threadIdx.x; idx < ny * W; idx += blockDim.x) {
@@ -463,7 +470,7 @@ __global__ void k_to_logical(const typename cplx_of<T>::type *arr, typename cplx
 
 /* noise test hook: Philox words and z per logical mode */
 template <typename T>
-__global__ void k_debug_noise(const __grid_constant__ Program P, int field, unsigned long long step, uint32_t *bits,
+__global__ void k_debug_noise(const __grid_constant__ Program P, unsigned rep, int field, unsigned long long step, uint32_t *bits,
                               typename cplx_of<T>::type *z) {
   const long long total = (long long)P.nxh * P.n[1] * P.n[2];
   for (long long m = blockIdx.x * (long long)blockDim.x + threadIdx.x; m < total; m += (long long)gridDim.x * blockDim.x) {
@@ -472,10 +479,10 @@ __global__ void k_debug_noise(const __grid_constant__ Program P, int field, unsi
     const int k1 = (int)(rp % P.n[1]), k2 = (int)(rp / P.n[1]);
     if (bits) {
       uint32_t w[4];
-      noise_block(P, field, step, m, w);
+      noise_block(P, rep, field, step, m, w);
       bits[4 * m] = w[0]; bits[4 * m + 1] = w[1]; bits[4 * m + 2] = w[2]; bits[4 * m + 3] = w[3];
     }
-    if (z) z[m] = noise_z<T>(P, field, step, k0, k1, k2);
+    if (z) z[m] = noise_z<T>(P, rep, field, step, k0, k1, k2);
   }
 }
 
@@ -501,6 +508,7 @@ __global__ void __launch_bounds__(256) k_step1d(const __grid_constant__ Program 
   const int RS = P.nfac + P.ngrp;
   const int tid = threadIdx.x, nt = blockDim.x;
   const C zero = mk<C, T>((T)0, (T)0);
+  C *const st1 = A.state + (size_t)blockIdx.x * P.ndyn * A.M; /* one CTA per ensemble replica */
   for (long long st = 0; st < A.nsteps; ++st) {
     /* steps 1-3: factor operators, mask, C2R (imaginary row unused) */
     for (int idx = tid; idx < A.geo.npad * RS; idx += nt) sm[idx] = zero;
@@ -509,7 +517,7 @@ __global__ void __launch_bounds__(256) k_step1d(const __grid_constant__ Program 
       const ModeQ<T> mq = make_mode<T>(P, kx, 0, 0);
       C phi[PSS_P_MAX_DYN];
 #pragma unroll
-      for (int i = 0; i < PSS_P_MAX_DYN; ++i) phi[i] = (i < P.ndyn) ? A.state[(size_t)i * A.M + kx] : zero;
+      for (int i = 0; i < PSS_P_MAX_DYN; ++i) phi[i] = (i < P.ndyn) ? st1[(size_t)i * A.M + kx] : zero;
       for (int f = 0; f < P.nfac; ++f) {
         const DFactor &F = P.fac[f];
         if (!keep_axis(P.dealias, F.order, kx, nx)) continue;
@@ -547,7 +555,7 @@ __global__ void __launch_bounds__(256) k_step1d(const __grid_constant__ Program 
       const C *srow = sm + (size_t)geo_pad(A.geo, kx) * RS + P.nfac;
       C phi[PSS_P_MAX_DYN], out[PSS_P_MAX_DYN];
 #pragma unroll
-      for (int i = 0; i < PSS_P_MAX_DYN; ++i) phi[i] = (i < P.ndyn) ? A.state[(size_t)i * A.M + kx] : zero;
+      for (int i = 0; i < PSS_P_MAX_DYN; ++i) phi[i] = (i < P.ndyn) ? st1[(size_t)i * A.M + kx] : zero;
 #pragma unroll
       for (int i = 0; i < PSS_P_MAX_DYN; ++i) {
         out[i] = zero;
@@ -562,7 +570,7 @@ __global__ void __launch_bounds__(256) k_step1d(const __grid_constant__ Program 
           C num = mk<C, T>(phi[i].x + (T)P.dt * N.x, phi[i].y + (T)P.dt * N.y);
           if (d.noisy) {
             const T amp = noise_amp<T>(d, mq);
-            const C z = noise_z<T>(P, d.field_id, A.step0 + (unsigned long long)st, kx, 0, 0);
+            const C z = noise_z<T>(P, blockIdx.x, d.field_id, A.step0 + (unsigned long long)st, kx, 0, 0);
             num.x += amp * z.x;
             num.y += amp * z.y;
           }
@@ -574,7 +582,7 @@ __global__ void __launch_bounds__(256) k_step1d(const __grid_constant__ Program 
       }
 #pragma unroll
       for (int i = 0; i < PSS_P_MAX_DYN; ++i)
-        if (i < P.ndyn) A.state[(size_t)i * A.M + kx] = out[i];
+        if (i < P.ndyn) st1[(size_t)i * A.M + kx] = out[i];
     }
     __syncthreads();
   }

@@ -87,11 +87,17 @@ __device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t
 }
 
 /* counter = (m_lo, m_hi, step_lo, ((step_hi & 0xffff) << 16) | field), key = seed */
-__device__ __forceinline__ void noise_block(const Program &P, int field, unsigned long long step, long long m,
+/* replica r of an ensemble is the system with seed + r (pss_set_replicas) */
+__device__ __forceinline__ unsigned long long replica_seed(const Program &P, unsigned rep) {
+  return ((((unsigned long long)P.seed_hi) << 32) | (unsigned long long)P.seed_lo) + (unsigned long long)rep;
+}
+__device__ __forceinline__ void noise_block(const Program &P, unsigned rep, int field, unsigned long long step, long long m,
                                             uint32_t w[4]) {
+  const unsigned long long sd = replica_seed(P, rep);
   philox4x32_10((uint32_t)((unsigned long long)m & 0xffffffffu), (uint32_t)((unsigned long long)m >> 32),
                 (uint32_t)(step & 0xffffffffu),
-                (uint32_t)((((step >> 32) & 0xffffu) << 16) | ((uint32_t)field & 0xffffu)), P.seed_lo, P.seed_hi, w);
+                (uint32_t)((((step >> 32) & 0xffffu) << 16) | ((uint32_t)field & 0xffffu)), (uint32_t)(sd & 0xffffffffu),
+                (uint32_t)(sd >> 32), w);
 }
 
 __device__ __forceinline__ void gauss_pair(const uint32_t w[4], float &g1, float &g2) {
@@ -184,7 +190,7 @@ __device__ __forceinline__ float2 box_muller_half(uint32_t w0, uint32_t w1) {
 
 /* unit-variance Hermitian complex Gaussian at logical mode (k0,k1,k2)  (Eq. 16, 134) */
 template <typename T>
-__device__ __forceinline__ typename cplx_of<T>::type noise_z(const Program &P, int field, unsigned long long step,
+__device__ __forceinline__ typename cplx_of<T>::type noise_z(const Program &P, unsigned rep, int field, unsigned long long step,
                                                              int k0, int k1, int k2) {
   typedef typename cplx_of<T>::type C;
   const long long n1 = P.n[1], n2 = P.n[2], nxh = P.nxh;
@@ -193,14 +199,14 @@ __device__ __forceinline__ typename cplx_of<T>::type noise_z(const Program &P, i
   T g1, g2;
   const bool on_plane = (k0 == 0) || (2 * k0 == P.n[0]);
   if (!on_plane) {
-    noise_block(P, field, step, m, w);
+    noise_block(P, rep, field, step, m, w);
     gauss_pair(w, g1, g2);
     const T h = (T)0.70710678118654752440;
     return mk<C, T>(g1 * h, g2 * h);
   }
   const long long p1 = (n1 - k1) % n1, p2 = (n2 - k2) % n2;
   const long long mp = (p2 * n1 + p1) * nxh + k0;
-  noise_block(P, field, step, m < mp ? m : mp, w);
+  noise_block(P, rep, field, step, m < mp ? m : mp, w);
   gauss_pair(w, g1, g2);
   if (mp == m) return mk<C, T>(g1, (T)0);
   const T h = (T)0.70710678118654752440;
@@ -209,15 +215,16 @@ __device__ __forceinline__ typename cplx_of<T>::type noise_z(const Program &P, i
 
 /* fp32: the same stream through the lean path (two words, own ln/sin/cos) */
 template <>
-__device__ __forceinline__ float2 noise_z<float>(const Program &P, int field, unsigned long long step, int k0, int k1, int k2) {
+__device__ __forceinline__ float2 noise_z<float>(const Program &P, unsigned rep, int field, unsigned long long step, int k0, int k1, int k2) {
   const long long n1 = P.n[1], n2 = P.n[2], nxh = P.nxh;
   /* 32-bit index arithmetic whenever the half-spectrum has fewer than 2^31 modes */
   const bool small = (long long)P.nxh * P.n[1] * P.n[2] < 0x7fffffffLL;
   long long m = small ? (long long)(unsigned)(((unsigned)k2 * (unsigned)P.n[1] + (unsigned)k1) * (unsigned)P.nxh + (unsigned)k0)
                       : ((long long)k2 * n1 + k1) * nxh + k0;
+  const unsigned long long sd = replica_seed(P, rep);
   NoiseKey K;
-  K.k0 = P.seed_lo;
-  K.k1 = P.seed_hi;
+  K.k0 = (uint32_t)(sd & 0xffffffffu);
+  K.k1 = (uint32_t)(sd >> 32);
   K.c2 = (uint32_t)(step & 0xffffffffu);
   K.c3 = (uint32_t)((((step >> 32) & 0xffffu) << 16) | ((uint32_t)field & 0xffffu));
   const bool on_plane = (k0 == 0) || (2 * k0 == P.n[0]);
