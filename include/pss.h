@@ -84,7 +84,7 @@ int pss_set_dealias(pss_system *, int rule);
 /* Ensemble (stochastic studies need many realisations): the system holds
  * `nreplicas` independent realisations of the same field system and pss_step advances all of them in the same
  * launches (grid dimension y).  Replica r is, bit for bit, the system created with seed + r.  Call before
- * pss_finalize; 1 <= nreplicas <= 65535.  The persistent 1024^2 kernel is used for nreplicas == 1 only. */
+ * pss_finalize; 1 <= nreplicas <= 65535.  The persistent 1024^2 kernel runs the replicas one launch after the other. */
 int pss_set_replicas(pss_system *, int nreplicas);
 /* which replica pss_set_field / pss_get_field / pss_get_field_fourier / pss_debug_noise address (default 0) */
 int pss_select_replica(pss_system *, int replica);

@@ -366,7 +366,7 @@ bool real_op(const DOp &d) { return ((d.a[0] + d.a[1] + d.a[2]) & 1) == 0; }
 bool fused2d_eligible(const pss_system *s) {
   const Program &P = s->P;
   if (env_int("PSS_FUSED", 1) == 0) return false;
-  if (s->ndim != 2 || s->prec != PSS_F32 || s->n[0] != f2d::N || s->n[1] != f2d::N || s->nrep != 1) return false;
+  if (s->ndim != 2 || s->prec != PSS_F32 || s->n[0] != f2d::N || s->n[1] != f2d::N) return false;
   if (P.ndyn != 1 || P.nfac != 1 || P.ngrp != 1) return false;
   if (P.dyn[0].lin_beg != P.dyn[0].lin_end) return false;
   if (!real_op(P.grp[0].outer)) return false;
@@ -631,24 +631,32 @@ template <typename T> int launch_rows(pss_system *s) {
 
 /* nsteps steps (plus the E-rebuilding prologue when the state was just set) in one cooperative launch */
 int launch_fused(pss_system *s, int64_t nsteps) {
-  f2d::Args a;
-  a.state = carr<float>(s, s->off_state, 0);
-  a.E = carr<float>(s, s->off_psix, 0);
-  a.Z = carr<float>(s, s->off_phat, 0);
-  a.tw = twp<float>(s, 0);
-  a.bar = reinterpret_cast<unsigned long long *>(s->ws + s->off_bar);
-  a.bar_base = s->bar_count;
-  a.nsteps = nsteps;
-  a.step0 = s->step;
-  a.prologue = s->psix_valid ? 0 : 1;
-  void *params[2] = {(void *)&s->P, (void *)&a};
+  const int prologue = s->psix_valid ? 0 : 1;
   const void *fn = s->plan.fused_prune ? (const void *)f2d::k_fused2d<true> : (const void *)f2d::k_fused2d<false>;
-  prof_mark(s, KIND_FUSED, true);
-  cudaError_t e = cudaLaunchCooperativeKernel(fn, dim3(f2d::NCTA), dim3(f2d::THREADS), params, f2d::SMEM_BYTES, s->stream);
-  prof_mark(s, KIND_FUSED, false);
-  if (e != cudaSuccess) return cuda_fail(s, e, "k_fused2d");
-  CKL("k_fused2d");
-  s->bar_count += (unsigned long long)f2d::NCTA * (unsigned long long)(2 * nsteps + a.prologue);
+  /* an ensemble runs its replicas one launch after the other (replica r: arrays [r], seed + r) */
+  for (int r = 0; r < s->nrep; ++r) {
+    Program Pr = s->P;
+    const uint64_t sd = s->seed + (uint64_t)r;
+    Pr.seed_lo = (uint32_t)(sd & 0xffffffffu);
+    Pr.seed_hi = (uint32_t)(sd >> 32);
+    f2d::Args a;
+    a.state = carr<float>(s, s->off_state, r * Pr.ndyn);
+    a.E = carr<float>(s, s->off_psix, r * Pr.nfac);
+    a.Z = carr<float>(s, s->off_phat, r * Pr.ngrp);
+    a.tw = twp<float>(s, 0);
+    a.bar = reinterpret_cast<unsigned long long *>(s->ws + s->off_bar);
+    a.bar_base = s->bar_count;
+    a.nsteps = nsteps;
+    a.step0 = s->step;
+    a.prologue = prologue;
+    void *params[2] = {(void *)&Pr, (void *)&a};
+    prof_mark(s, KIND_FUSED, true);
+    cudaError_t e = cudaLaunchCooperativeKernel(fn, dim3(f2d::NCTA), dim3(f2d::THREADS), params, f2d::SMEM_BYTES, s->stream);
+    prof_mark(s, KIND_FUSED, false);
+    if (e != cudaSuccess) return cuda_fail(s, e, "k_fused2d");
+    CKL("k_fused2d");
+    s->bar_count += (unsigned long long)f2d::NCTA * (unsigned long long)(2 * nsteps + prologue);
+  }
   s->psix_valid = true;
   s->step += (uint64_t)nsteps;
   return PSS_OK;
