@@ -101,10 +101,10 @@ __device__ __forceinline__ float2 cmulf(float2 a, float2 w) {
 
 /* 4-point forward DFT, natural in, natural out */
 __device__ __forceinline__ void dft4(float2 &x0, float2 &x1, float2 &x2, float2 &x3) {
-  const float2 s02 = make_float2(x0.x + x2.x, x0.y + x2.y), d02 = make_float2(x0.x - x2.x, x0.y - x2.y);
-  const float2 s13 = make_float2(x1.x + x3.x, x1.y + x3.y), d13 = make_float2(x1.x - x3.x, x1.y - x3.y);
-  x0 = make_float2(s02.x + s13.x, s02.y + s13.y);
-  x2 = make_float2(s02.x - s13.x, s02.y - s13.y);
+  const float2 s02 = cadd(x0, x2), d02 = csub(x0, x2);
+  const float2 s13 = cadd(x1, x3), d13 = csub(x1, x3);
+  x0 = cadd(s02, s13);
+  x2 = csub(s02, s13);
   x1 = make_float2(d02.x + d13.y, d02.y - d13.x); /* d02 - i d13 */
   x3 = make_float2(d02.x - d13.y, d02.y + d13.x); /* d02 + i d13 */
 }
