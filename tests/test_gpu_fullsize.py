@@ -133,3 +133,64 @@ def test_fullsize_step_splitting_is_bit_identical(pss):
     assert np.array_equal(a.get_field_fourier(f).view(np.uint32), b.get_field_fourier(f).view(np.uint32))
     m = a.get_field_fourier(f)[0, 0]
     assert m.imag == 0.0
+
+
+# ---------------------------------------------------------------------------------------------
+# properties that hold at any size, checked on the CUDA path alone at the headline size
+# ---------------------------------------------------------------------------------------------
+def test_config2_full_run_conserves_mass_and_phase_separates(pss):
+    """config 2 in full: 10^4 steps of the headline workload in the launch configuration bench.py times.
+    Conserved dynamics keep the q = 0 mode bit-identical (P5); the off-critical quench coarsens towards the
+    phases +-sqrt(-a/b) = +-1 and stays finite."""
+    cfg = wl.make_config("modelb_1024")
+    g, ids = wl.build(pss, cfg, prec="f32")
+    f = ids["phi"]
+    m0 = g.get_field_fourier(f)[0, 0]
+    v0 = float(np.var(g.get_field(f)))
+    g.step(5000)
+    g.step(5000)
+    assert g.step_count == 10000 and g.uses_fused_kernel
+    spec = g.get_field_fourier(f)
+    assert spec[0, 0].real == m0.real and spec[0, 0].imag == 0.0
+    x = g.get_field(f).astype(np.float64)
+    assert np.all(np.isfinite(x))
+    assert abs(x.mean() - 0.1) < 1e-5
+    assert np.var(x) > 50 * v0 and np.abs(x).max() < 1.5      # domains have formed, amplitudes bounded by the phases
+    assert np.mean(x > 0.5) > 0.3                             # majority phase near +1 (mean 0.1)
+
+
+def test_fused_kernel_stationary_structure_factor(pss):
+    """oracle-independent pin of the noise amplitude and Hermitian rule of the persistent kernel (A1, P6):
+    linear conserved dynamics d phi = -(a q^2 + k q^4) phi + noise D q^2 at 1024^2; the stationary
+    <|phi_q|^2> = (N/dV) 2 D q^2 / (lam (2 + dt lam)), lam = a q^2 + k q^4, averaged over many modes."""
+    n, dt, a, k, D = 1024, 0.05, 1.0, 1.0, 0.02
+    s = pss.System((n, n), (1.0, 1.0), dt, prec="f32", seed=31337)
+    f = s.add_field("phi", True)
+    s.add_linear(f, {"coef": a, "q2_pow": 1})
+    s.add_linear(f, {"coef": k, "q2_pow": 2})
+    s.add_term(f, {"coef": 0.0, "q2_pow": 1}, [f, f, f])      # a product group with zero weight: fused-kernel eligible
+    s.set_noise(f, D, 2)
+    s.finalize()
+    assert s.uses_fused_kernel
+    s.set_field(f, np.zeros((n, n), np.float32))
+    ky = np.fft.fftfreq(n, 1.0 / n)[:, None]
+    kx = np.arange(n // 2 + 1)[None, :]
+    q2 = (2 * np.pi / n) ** 2 * (kx ** 2 + ky ** 2)
+    lam = a * q2 + k * q2 ** 2
+    with np.errstate(divide="ignore", invalid="ignore"):
+        S_th = n * n * 2 * D * q2 / (lam * (2 + dt * lam))
+    sel = (q2 > 0.5) & (kx > 0) & (kx < n // 2)               # relaxation time 1/lam < 2: decorrelated between samples
+    s.step(400)
+    acc, cnt = np.zeros_like(q2), 0
+    for _ in range(12):
+        s.step(100)
+        spec = s.get_field_fourier(f)
+        acc += np.abs(spec.astype(np.complex128)) ** 2
+        cnt += 1
+    ratio = (acc / cnt)[sel] / S_th[sel]
+    assert abs(ratio.mean() - 1.0) < 0.01, ratio.mean()       # ~3e5 modes x 12 samples
+    # boundary planes kx = 0 and kx = n/2 carry the same variance (Hermitian rule)
+    for col in (0, n // 2):
+        m = (q2[:, col] > 0.5)
+        r = (acc / cnt)[m, col] / S_th[m, col]
+        assert abs(r.mean() - 1.0) < 0.08, (col, r.mean())
