@@ -41,6 +41,7 @@ struct Plan {
   int kx_keep_max;                  /* max over factors of the number of kept kx */
   int fused;                        /* 1: the persistent 1024^2 fp32 kernel of pss_fused2d.cuh runs the steps (PSS_FUSED=0 disables) */
   int fused_prune;                  /* its input-pruned instantiation (mask cutoff <= n/4 on both axes)       */
+  int fused_pair;                   /* ensembles: two replicas per launch (k_fused2d_pair)                    */
 };
 
 }  // namespace
@@ -527,6 +528,18 @@ int setup_fused(pss_system *s) {
   else
     CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, f2d::k_fused2d<false>, f2d::THREADS, f2d::SMEM_BYTES));
   if (!coop || (long long)occ * nsm < f2d::NCTA) s->plan.fused = 0;
+  /* ensembles: the two-replica kernel needs more shared memory; fall back to one launch per replica if it does not fit */
+  s->plan.fused_pair = 0;
+  if (s->plan.fused && s->nrep >= 2 && env_int("PSS_FUSED_PAIR", 1) != 0) {
+    int occ2 = 0;
+    CK(cudaFuncSetAttribute(f2d::k_fused2d_pair<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)f2d::SMEM_BYTES_PAIR));
+    CK(cudaFuncSetAttribute(f2d::k_fused2d_pair<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)f2d::SMEM_BYTES_PAIR));
+    if (s->plan.fused_prune)
+      CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ2, f2d::k_fused2d_pair<true>, f2d::THREADS, f2d::SMEM_BYTES_PAIR));
+    else
+      CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ2, f2d::k_fused2d_pair<false>, f2d::THREADS, f2d::SMEM_BYTES_PAIR));
+    if ((long long)occ2 * nsm >= f2d::NCTA) s->plan.fused_pair = 1;
+  }
   return PSS_OK;
 }
 
@@ -632,9 +645,12 @@ template <typename T> int launch_rows(pss_system *s) {
 /* nsteps steps (plus the E-rebuilding prologue when the state was just set) in one cooperative launch */
 int launch_fused(pss_system *s, int64_t nsteps) {
   const int prologue = s->psix_valid ? 0 : 1;
-  const void *fn = s->plan.fused_prune ? (const void *)f2d::k_fused2d<true> : (const void *)f2d::k_fused2d<false>;
-  /* an ensemble runs its replicas one launch after the other (replica r: arrays [r], seed + r) */
-  for (int r = 0; r < s->nrep; ++r) {
+  const void *fn1 = s->plan.fused_prune ? (const void *)f2d::k_fused2d<true> : (const void *)f2d::k_fused2d<false>;
+  const void *fn2 = s->plan.fused_prune ? (const void *)f2d::k_fused2d_pair<true> : (const void *)f2d::k_fused2d_pair<false>;
+  /* an ensemble runs its replicas two per launch (k_fused2d_pair overlaps one replica's L2 exchanges with the
+   * other's transforms), a last odd one alone; replica r: arrays [r], seed + r */
+  for (int r = 0; r < s->nrep;) {
+    const bool pair = s->plan.fused_pair && r + 1 < s->nrep;
     Program Pr = s->P;
     const uint64_t sd = s->seed + (uint64_t)r;
     Pr.seed_lo = (uint32_t)(sd & 0xffffffffu);
@@ -649,13 +665,16 @@ int launch_fused(pss_system *s, int64_t nsteps) {
     a.nsteps = nsteps;
     a.step0 = s->step;
     a.prologue = prologue;
+    a.rep_stride = arr_stride(s); /* ndyn = nfac = ngrp = 1: consecutive replicas are one array apart */
     void *params[2] = {(void *)&Pr, (void *)&a};
     prof_mark(s, KIND_FUSED, true);
-    cudaError_t e = cudaLaunchCooperativeKernel(fn, dim3(f2d::NCTA), dim3(f2d::THREADS), params, f2d::SMEM_BYTES, s->stream);
+    cudaError_t e = cudaLaunchCooperativeKernel(pair ? fn2 : fn1, dim3(f2d::NCTA), dim3(f2d::THREADS), params,
+                                                pair ? f2d::SMEM_BYTES_PAIR : f2d::SMEM_BYTES, s->stream);
     prof_mark(s, KIND_FUSED, false);
     if (e != cudaSuccess) return cuda_fail(s, e, "k_fused2d");
     CKL("k_fused2d");
     s->bar_count += (unsigned long long)f2d::NCTA * (unsigned long long)(2 * nsteps + prologue);
+    r += pair ? 2 : 1;
   }
   s->psix_valid = true;
   s->step += (uint64_t)nsteps;

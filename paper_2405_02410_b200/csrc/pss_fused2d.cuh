@@ -61,6 +61,7 @@ struct Args {
   long long nsteps;
   unsigned long long step0;
   int prologue;                  /* 1: E is stale (after pss_set_field): rebuild it from the state first */
+  long long rep_stride;          /* k_fused2d_pair: elements between the arrays of replica r and r+1 (state, E, Z alike) */
 };
 
 __device__ __forceinline__ float2 ldcg2(const float2 *p) { return __ldcg(p); }
@@ -398,6 +399,244 @@ __global__ void __launch_bounds__(THREADS, 1) k_fused2d(const __grid_constant__ 
   if (colw && A.nsteps > 0) {
 #pragma unroll
     for (int r = 0; r < 16; ++r) A.state[(size_t)kx * N + kyb + 16 * (r & 3) + 256 * (r >> 2)] = st[r];
+  }
+}
+
+/* ------------------------------------------------------------------------------------------ */
+/* TWO ensemble replicas (seed, seed + 1; pss_set_replicas) in one persistent launch.  A single system cannot
+ * overlap its two bulk-synchronous L2 exchanges with anything but the noise; two independent replicas can: the
+ * loads of replica 1 are in flight while replica 0 is transformed, the stores of replica 0 drain while replica 1
+ * is transformed, and each grid barrier is paid once per two replica-steps.  Per replica the arithmetic is exactly
+ * that of k_fused2d (bit-identical results).  Differences in storage: the states live in shared memory (the
+ * registers hold the prefetched loads instead) and z is single-buffered per replica. */
+constexpr int NRE = 2;
+constexpr size_t SMEM_BYTES_PAIR = (size_t)(4 * BUF + 2 * NRE * 16 * TT) * sizeof(float2) + (size_t)16 * TT * sizeof(float4);
+
+template <bool PRUNE>
+__global__ void __launch_bounds__(THREADS, 1) k_fused2d_pair(const __grid_constant__ Program P, const Args A) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  float2 *xs = reinterpret_cast<float2 *>(smem_raw);                  /* [4][BUF] exchange buffers            */
+  float2 *zbuf = xs + 4 * BUF;                                        /* [NRE][16 r][256 tid] unit noise z    */
+  float2 *stS = zbuf + NRE * 16 * TT;                                 /* [NRE][16 r][256 tid] state phi_q     */
+  float4 *tab = reinterpret_cast<float4 *>(stS + NRE * 16 * TT);      /* [16 r][256 tid] per-mode coefficients */
+
+  const int tid = threadIdx.x & (TT - 1);
+  const bool noisew = threadIdx.x >= TT;
+  const int L = tid & 3, tq = tid >> 2;
+  const int b = blockIdx.x;
+  int kx;
+  if (b < 128) kx = (L < 2) ? (2 * b + L) : (256 + 2 * b + (L - 2));
+  else kx = (L == 0) ? 512 : -1;
+  const bool colw = kx >= 0;
+  const int kxm = colw ? ((N - kx) & (N - 1)) : 0;
+  const bool selfc = (kx == 0) || (kx == 512);
+  const int kyb = (tq & 15) + 64 * (tq >> 4);
+  const DDyn &D0 = P.dyn[0];
+  const bool noisy = D0.noisy != 0;
+
+  if (noisew) {
+    asm volatile("setmaxnreg.dec.sync.aligned.u32 64;");
+    if (!noisy || A.nsteps <= 0) return;
+    const unsigned long long sd0 = (((unsigned long long)P.seed_hi) << 32) | (unsigned long long)P.seed_lo;
+#pragma unroll 1
+    for (long long s = 0; s < A.nsteps; ++s) {
+      const unsigned long long step = A.step0 + (unsigned long long)s;
+#pragma unroll 1
+      for (int r = 0; r < NRE; ++r) {
+        NoiseKey K;
+        const unsigned long long sd = sd0 + (unsigned long long)r;
+        K.k0 = (uint32_t)(sd & 0xffffffffu);
+        K.k1 = (uint32_t)(sd >> 32);
+        K.c2 = (uint32_t)(step & 0xffffffffu);
+        K.c3 = (uint32_t)((((step >> 32) & 0xffffu) << 16) | ((uint32_t)D0.field_id & 0xffffu));
+        if (s >= 1) nb_sync(4 + r); /* the transform warps have consumed z_r(s-1) */
+        if (colw) {
+          float2 *zw = zbuf + (size_t)r * 16 * TT + tid;
+#pragma unroll 2
+          for (int i = 0; i < 16; ++i)
+            zw[i * TT] = noise_mode(K, kx, kyb + 16 * (i & 3) + 256 * (i >> 2), selfc);
+        }
+        nb_arrive(2 + r);
+      }
+    }
+    return;
+  }
+
+  asm volatile("setmaxnreg.inc.sync.aligned.u32 184;");
+  const bool need_inv = colw && keep_axis(P.dealias, P.fac[0].order, kx, N);
+  const bool roww = b < 128;
+  Lane ln;
+  ln.xl = xs + L * BUF;
+  ln.tq = tq;
+#pragma unroll
+  for (int i = 0; i < 16; ++i) {
+    ln.t1[i] = A.tw[(i * tq) & (N - 1)];
+    ln.t2[i] = A.tw[(16 * i * (tq & 3)) & (N - 1)];
+  }
+  {
+    const float dt = (float)P.dt, invN = (float)P.invN;
+#pragma unroll 1
+    for (int i = 0; i < 16; ++i) {
+      float4 t = make_float4(0.f, 0.f, 0.f, 0.f);
+      const int ky = kyb + 16 * (i & 3) + 256 * (i >> 2);
+      if (colw) {
+        const ModeQ<float> mq = make_mode<float>(P, kx, ky, 0);
+        t.x = dt * eval_op<float>(P.grp[0].outer, mq).x;
+        float Lq = 0.f;
+        for (int e = D0.lhs_beg; e < D0.lhs_end; ++e) Lq -= eval_op<float>(P.lin[e], mq).x;
+        t.y = 1.0f / (1.0f - dt * Lq);
+        t.z = noisy ? noise_amp<float>(D0, mq) : 0.f;
+        float fc = 0.f;
+        if (need_inv && keep_axis(P.dealias, P.fac[0].order, ky, N)) {
+          for (int e = P.fac[0].lin_beg; e < P.fac[0].lin_end; ++e) fc += eval_op<float>(P.lin[e], mq).x;
+          fc *= invN;
+        }
+        t.w = fc;
+      }
+      tab[i * TT + tid] = t;
+      for (int r = 0; r < NRE; ++r) {
+        stS[(size_t)r * 16 * TT + i * TT + tid] =
+            colw ? A.state[(size_t)r * A.rep_stride + (size_t)kx * N + ky] : make_float2(0.f, 0.f);
+        if (!noisy) zbuf[(size_t)r * 16 * TT + i * TT + tid] = make_float2(0.f, 0.f);
+      }
+    }
+  }
+  float c2 = 0.f, c3 = 0.f, c4 = 0.f;
+  for (int t = P.grp[0].term_beg; t < P.grp[0].term_end; ++t) {
+    const float c = (float)P.term[t].coef;
+    if (P.term[t].nf == 2) c2 += c;
+    else if (P.term[t].nf == 3) c3 += c;
+    else c4 += c;
+  }
+  unsigned long long bar_target = A.bar_base;
+  const long long nphase = A.nsteps + (A.prologue ? 1 : 0);
+  tsync();
+
+  float2 v[16], nx[16];
+#pragma unroll 1
+  for (long long it = 0; it < nphase; ++it) {
+    const bool pro = A.prologue && it == 0;
+    const long long ls = it - (A.prologue ? 1 : 0);
+    /* ph = 0: rows (inverse-x, product, forward-x)   ph = 1: columns (forward-y, Eq. 15/16/18, inverse-y) */
+#pragma unroll 1
+    for (int ph = pro ? 1 : 0; ph < 2; ++ph) {
+#pragma unroll 1
+      for (int r = 0; r <= NRE; ++r) {
+        /* software pipeline: issue the loads of replica r (into nx) before transforming replica r - 1 (in v) */
+        const bool have_prev = r > 0;
+        if (have_prev) {
+          /* nx holds the raw loads of replica r - 1: turn them into the transform input */
+          if (ph == 0) {
+#pragma unroll
+            for (int i = 0; i < 16; ++i) v[i] = make_float2(nx[i].x, -nx[i].y);
+          } else if (!pro) {
+#pragma unroll
+            for (int a = 0; a < 8; ++a) {
+              const float2 za = nx[a], zc = nx[a + 8];
+              v[a] = make_float2(0.5f * (za.x + zc.x), 0.5f * (za.y - zc.y));
+              v[a + 8] = make_float2(0.5f * (za.y + zc.y), 0.5f * (zc.x - za.x));
+            }
+          }
+        }
+        if (r < NRE && !pro) {
+          if (ph == 0) {
+            if (roww) {
+              const float2 *Eb = A.E + (size_t)r * A.rep_stride + ((size_t)b * N) * 4 + L + (size_t)kyb * 4;
+#pragma unroll
+              for (int i = 0; i < 16; ++i) {
+                if (!PRUNE || (i >> 2) == 0 || (i >> 2) == 3) nx[i] = ldcg2(Eb + (size_t)(16 * (i & 3) + 256 * (i >> 2)) * 4);
+                else nx[i] = make_float2(0.f, 0.f);
+              }
+            } else {
+#pragma unroll
+              for (int i = 0; i < 16; ++i) nx[i] = make_float2(0.f, 0.f);
+            }
+          } else {
+            if (colw) {
+              const float2 *Z1 = A.Z + (size_t)r * A.rep_stride + (size_t)kx * NP + tq;
+              const float2 *Z2 = A.Z + (size_t)r * A.rep_stride + (size_t)kxm * NP + tq;
+#pragma unroll
+              for (int a = 0; a < 8; ++a) { nx[a] = ldcg2(Z1 + 64 * a); nx[a + 8] = ldcg2(Z2 + 64 * a); }
+            } else {
+#pragma unroll
+              for (int a = 0; a < 16; ++a) nx[a] = make_float2(0.f, 0.f);
+            }
+          }
+        }
+        if (!have_prev) continue;
+        const int rr = r - 1; /* the replica being transformed */
+        float2 *myst = stS + (size_t)rr * 16 * TT + tid;
+        if (ph == 0) {
+          fwd_dit(v, ln);
+#pragma unroll
+          for (int a = 0; a < 16; ++a) {
+            const float ra = v[a].x, rb = -v[a].y;
+            v[a] = make_float2(ra * ra * (c2 + ra * (c3 + ra * c4)), rb * rb * (c2 + rb * (c3 + rb * c4)));
+          }
+          tsync();
+          fwd_dif(v, ln);
+          if (roww) {
+            float2 *Zb = A.Z + (size_t)rr * A.rep_stride + (size_t)kyb * NP + 4 * b + L;
+#pragma unroll
+            for (int i = 0; i < 16; ++i) Zb[(size_t)(16 * (i & 3) + 256 * (i >> 2)) * NP] = v[i];
+          }
+          tsync();
+        } else {
+          if (!pro) {
+            fwd_dif(v, ln);
+            if (noisy) nb_sync(2 + rr);
+            const float2 *myz = zbuf + (size_t)rr * 16 * TT + tid;
+#pragma unroll
+            for (int i = 0; i < 16; ++i) {
+              const float4 tt = tab[i * TT + tid];
+              const float2 z = myz[i * TT];
+              const float2 pq = v[i];
+              const float2 so = myst[i * TT];
+              const float nxr = (so.x + tt.x * pq.x) + tt.z * z.x;
+              const float nyr = (so.y + tt.x * pq.y) + tt.z * z.y;
+              const float2 sn = make_float2(nxr * tt.y, nyr * tt.y);
+              myst[i * TT] = sn;
+              v[i] = make_float2(sn.x * tt.w, -sn.y * tt.w);
+            }
+            if (noisy && ls + 1 < A.nsteps) nb_arrive(4 + rr);
+            tsync();
+          } else {
+#pragma unroll
+            for (int i = 0; i < 16; ++i) {
+              const float fc = tab[i * TT + tid].w;
+              const float2 so = myst[i * TT];
+              v[i] = make_float2(so.x * fc, -so.y * fc);
+            }
+          }
+          fwd_dit(v, ln);
+          if (need_inv) {
+#pragma unroll
+            for (int a = 0; a < 8; ++a) {
+              const float2 av = make_float2(v[a].x, -v[a].y);
+              const float2 bv = make_float2(v[a + 8].x, -v[a + 8].y);
+              const int p = 64 * a + tq;
+              float2 *e = A.E + (size_t)rr * A.rep_stride + ((size_t)(p >> 2) * N) * 4 + (p & 3);
+              if (selfc) {
+                e[(size_t)kx * 4] = make_float2(av.x, bv.x);
+              } else {
+                e[(size_t)kx * 4] = make_float2(av.x - bv.y, av.y + bv.x);
+                e[(size_t)kxm * 4] = make_float2(av.x + bv.y, bv.x - av.y);
+              }
+            }
+          }
+          tsync();
+        }
+      }
+      bar_target += NCTA;
+      grid_barrier(A.bar, bar_target);
+    }
+  }
+
+  if (colw && A.nsteps > 0) {
+    for (int r = 0; r < NRE; ++r)
+#pragma unroll
+      for (int i = 0; i < 16; ++i)
+        A.state[(size_t)r * A.rep_stride + (size_t)kx * N + kyb + 16 * (i & 3) + 256 * (i >> 2)] = stS[(size_t)r * 16 * TT + i * TT + tid];
   }
 }
 
