@@ -323,6 +323,15 @@ int build_program(pss_system *s) {
 }
 
 /* ---- launch plan ----------------------------------------------------------------------- */
+/* entries of one axis' twiddle array: tw[n] followed by the per-pass tables (Geo::twoff) */
+long long tw_entries(const Geo &g) {
+  long long e = g.n;
+  int lgL = 0;
+  for (int q = 0; q < g.nr; ++q) lgL += g.lg[q];
+  for (int q = 0; q < g.nr; ++q) { e += (long long)((1 << g.lg[q]) - 1) << (lgL - g.lg[q]); lgL -= g.lg[q]; }
+  return e;
+}
+
 int geo_pad_h(const Geo &g, int p) { return p + (p >> g.sh[0]) + (p >> g.sh[1]) + (p >> g.sh[2]); }
 
 Geo make_geo(int64_t n) {
@@ -347,6 +356,14 @@ Geo make_geo(int64_t n) {
       fs += g.lg[q];
     } else {
       g.fs[q] = 0; g.ps[q] = 0; g.fm[q] = 0;
+    }
+  }
+  {
+    long long off = n;
+    int lgL = lg;
+    for (int q = 0; q < 4; ++q) {
+      g.twoff[q] = (int32_t)off;
+      if (q < np) { off += (long long)((1 << g.lg[q]) - 1) << (lgL - g.lg[q]); lgL -= g.lg[q]; }
     }
   }
   return g;
@@ -482,7 +499,7 @@ void carve_workspace(pss_system *s) {
   s->off_phat = off;  off += arr * (size_t)(P.ngrp > 0 ? P.ngrp : 0) * R;
   s->off_scratch = off; off += arr;
   s->off_ureal = off; off += align_up((size_t)s->N * s->rsize, 256);
-  for (int j = 0; j < 3; ++j) { s->off_tw[j] = off; off += align_up((size_t)s->n[j] * s->csize, 256); }
+  for (int j = 0; j < 3; ++j) { s->off_tw[j] = off; off += align_up((size_t)tw_entries(s->plan.geo[j]) * s->csize, 256); }
   s->off_bar = off; off += 256;
   s->ws_need = off;
 }
@@ -552,6 +569,19 @@ template <typename T> int upload_twiddles(pss_system *s) {
       const long double a = 2.0L * PI_L * (long double)i / (long double)s->n[j];
       tw[(size_t)i].x = (T)cosl(a);
       tw[(size_t)i].y = (T)(-sinl(a));
+    }
+    /* per-pass tables: the same numbers, re-ordered so that consecutive butterflies read consecutive entries */
+    const Geo &g = s->plan.geo[j];
+    int lgn = 0;
+    for (int q = 0; q < g.nr; ++q) lgn += g.lg[q];
+    tw.resize((size_t)tw_entries(g));
+    int lgL = lgn;
+    for (int q = 0; q < g.nr; ++q) {
+      const int R = 1 << g.lg[q], lgLs = lgL - g.lg[q];
+      for (int m = 1; m < R; ++m)
+        for (int i = 0; i < (1 << lgLs); ++i)
+          tw[(size_t)g.twoff[q] + ((size_t)(m - 1) << lgLs) + i] = tw[((size_t)m * i) << (lgn - lgL)];
+      lgL -= g.lg[q];
     }
     CK(cudaMemcpyAsync(s->ws + s->off_tw[j], tw.data(), tw.size() * sizeof(C), cudaMemcpyHostToDevice, s->stream));
     CK(cudaStreamSynchronize(s->stream)); /* tw is a stack-lifetime host buffer */

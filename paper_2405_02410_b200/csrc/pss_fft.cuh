@@ -148,7 +148,7 @@ __device__ __forceinline__ int geo_rev_fast(const Geo &g, int p) {
  * DIT = false: butterfly then twiddle (DIF).  DIT = true: twiddle then butterfly. */
 template <int LGR, int SGN, bool DIT, typename T>
 __device__ __forceinline__ void fft_pass(const Geo &g, typename cplx_of<T>::type *buf, const typename cplx_of<T>::type *__restrict__ tw,
-                                         int lgn, int lgL, int ncol, int rs) {
+                                         int lgn, int lgL, int ncol, int rs, int twoff) {
   typedef typename cplx_of<T>::type C;
   constexpr int R = 1 << LGR;
   const int lgLs = lgL - LGR;          /* log2 of the leg stride L/R */
@@ -163,14 +163,14 @@ __device__ __forceinline__ void fft_pass(const Geo &g, typename cplx_of<T>::type
     const int i = b & ((1 << lgLs) - 1);
     const int blk = b >> lgLs;
     C *p = buf + (size_t)geo_pad(g, (blk << lgL) + i) * rs + c;
-    const int tws = i << (lgn - lgL);  /* twiddle index step: w_L^i = tw[i * n/L] */
+    const C *twp = tw + twoff + i;     /* w_L^(m i) at twp[(m - 1) << lgLs] */
     C v[R];
 #pragma unroll
     for (int k = 0; k < R; ++k) v[k] = p[k * ls];
     if (DIT && !notw) {
 #pragma unroll
       for (int m = 1; m < R; ++m) {
-        const C w = __ldg(tw + m * tws);
+        const C w = __ldg(twp + ((m - 1) << lgLs));
         v[m] = (SGN < 0) ? cmul(v[m], w) : cmulc(v[m], w);
       }
     }
@@ -178,7 +178,7 @@ __device__ __forceinline__ void fft_pass(const Geo &g, typename cplx_of<T>::type
     if (!DIT && !notw) {
 #pragma unroll
       for (int m = 1; m < R; ++m) {
-        const C w = __ldg(tw + m * tws);
+        const C w = __ldg(twp + ((m - 1) << lgLs));
         v[m] = (SGN < 0) ? cmul(v[m], w) : cmulc(v[m], w);
       }
     }
@@ -189,12 +189,12 @@ __device__ __forceinline__ void fft_pass(const Geo &g, typename cplx_of<T>::type
 
 template <int SGN, bool DIT, typename T>
 __device__ __forceinline__ void fft_pass_any(const Geo &g, int lgr, typename cplx_of<T>::type *buf,
-                                             const typename cplx_of<T>::type *__restrict__ tw, int lgn, int lgL, int ncol, int rs) {
+                                             const typename cplx_of<T>::type *__restrict__ tw, int lgn, int lgL, int ncol, int rs, int twoff) {
   switch (lgr) {
-    case 1: fft_pass<1, SGN, DIT, T>(g, buf, tw, lgn, lgL, ncol, rs); break;
-    case 2: fft_pass<2, SGN, DIT, T>(g, buf, tw, lgn, lgL, ncol, rs); break;
-    case 3: fft_pass<3, SGN, DIT, T>(g, buf, tw, lgn, lgL, ncol, rs); break;
-    default: fft_pass<4, SGN, DIT, T>(g, buf, tw, lgn, lgL, ncol, rs); break;
+    case 1: fft_pass<1, SGN, DIT, T>(g, buf, tw, lgn, lgL, ncol, rs, twoff); break;
+    case 2: fft_pass<2, SGN, DIT, T>(g, buf, tw, lgn, lgL, ncol, rs, twoff); break;
+    case 3: fft_pass<3, SGN, DIT, T>(g, buf, tw, lgn, lgL, ncol, rs, twoff); break;
+    default: fft_pass<4, SGN, DIT, T>(g, buf, tw, lgn, lgL, ncol, rs, twoff); break;
   }
 }
 
@@ -206,7 +206,7 @@ __device__ __forceinline__ void fft_dif(const Geo &g, typename cplx_of<T>::type 
   for (int q = 0; q < g.nr; ++q) lgn += g.lg[q];
   int lgL = lgn;
   for (int q = 0; q < g.nr; ++q) {
-    fft_pass_any<SGN, false, T>(g, g.lg[q], buf, tw, lgn, lgL, ncol, rs);
+    fft_pass_any<SGN, false, T>(g, g.lg[q], buf, tw, lgn, lgL, ncol, rs, g.twoff[q]);
     lgL -= g.lg[q];
     __syncthreads();
   }
@@ -221,7 +221,7 @@ __device__ __forceinline__ void fft_dit(const Geo &g, typename cplx_of<T>::type 
   int lgL = 0;
   for (int q = g.nr - 1; q >= 0; --q) {
     lgL += g.lg[q];
-    fft_pass_any<SGN, true, T>(g, g.lg[q], buf, tw, lgn, lgL, ncol, rs);
+    fft_pass_any<SGN, true, T>(g, g.lg[q], buf, tw, lgn, lgL, ncol, rs, g.twoff[q]);
     __syncthreads();
   }
 }

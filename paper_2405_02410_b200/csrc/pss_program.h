@@ -102,6 +102,10 @@ struct Geo {
   /* digit fields of the reversal: digit q of frequency f sits at bits [fs[q], fs[q]+lg[q]) and moves to slot bits
    * starting at ps[q]; fm[q] is its mask (0 for unused passes) */
   int32_t fs[4], ps[4], fm[4];
+  /* per-pass twiddle tables behind the n-entry table tw[j] = exp(-2 pi i j / n): pass q (sub-length L, radix R) finds
+   * w_L^(m i) at tw[twoff[q] + (m - 1) * (L / R) + i], m = 1..R-1, i < L/R — consecutive butterflies read consecutive
+   * entries (two cache lines per warp load instead of up to 32) */
+  int32_t twoff[4];
 };
 
 #endif
