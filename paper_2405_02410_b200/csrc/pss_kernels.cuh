@@ -19,6 +19,10 @@
 #define PSS_KERNELS_CUH
 #include "pss_pointwise.cuh"
 
+#ifndef PSS_MINB
+#define PSS_MINB 3 /* fp32 k_rows / k_update: resident CTAs per SM the register budget is tuned for */
+#endif
+
 template <typename T> struct UpdArgs {
   typename cplx_of<T>::type *state; /* [ndyn][M] */
   typename cplx_of<T>::type *psix;  /* [nfac][M] */
@@ -71,7 +75,7 @@ template <typename T> __device__ __forceinline__ T horner4(const T (&c)[5], T x)
 /* ------------------------------------------------------------------------------------------ */
 /* RAD: the "radial" fast path of pss_program.h (every per-mode coefficient is a polynomial in q^2) */
 template <typename T, bool RAD>
-__global__ void __launch_bounds__(256, sizeof(T) == 4 ? 3 : 2) k_update(const __grid_constant__ Program P, const UpdArgs<T> A) {
+__global__ void __launch_bounds__(256, sizeof(T) == 4 ? PSS_MINB : 2) k_update(const __grid_constant__ Program P, const UpdArgs<T> A) {
   typedef typename cplx_of<T>::type C;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   C *sm = reinterpret_cast<C *>(smem_raw);
@@ -259,7 +263,7 @@ template <typename T> struct RowArgs {
 
 /* BIG: one CTA per SM (tile > half of the shared memory): 512 threads, else 256 threads and 3 CTAs per SM */
 template <typename T, bool BIG>
-__global__ void __launch_bounds__(BIG ? 512 : 256, (!BIG && sizeof(T) == 4) ? 3 : 1) k_rows(const __grid_constant__ Program P, const RowArgs<T> A) {
+__global__ void __launch_bounds__(BIG ? 512 : 256, (!BIG && sizeof(T) == 4) ? PSS_MINB : 1) k_rows(const __grid_constant__ Program P, const RowArgs<T> A) {
   typedef typename cplx_of<T>::type C;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   C *sm = reinterpret_cast<C *>(smem_raw);
