@@ -226,4 +226,106 @@ __device__ __forceinline__ void fft_dit(const Geo &g, typename cplx_of<T>::type 
   }
 }
 
+/* ---- first DIF pass fed straight from global memory / last DIT pass written straight to global memory ----
+ * The outermost pass (sub-length L = n) touches legs j = k*(n/R) + i: with the butterfly index i fastest across the
+ * threads, leg k of a warp is one contiguous run in the line, so the pass can take its input from (or deliver its
+ * output to) global memory directly and the separate copy loop and its barrier disappear.
+ *   load(cc, j)       -> element j of column cc        store(cc, j, v): element j (natural order) of column cc */
+template <int LGR, int SGN, typename T, typename LD>
+__device__ __forceinline__ void fft_first_from(const Geo &g, typename cplx_of<T>::type *buf, const typename cplx_of<T>::type *__restrict__ tw,
+                                               int lgn, int ncol, int rs, LD load) {
+  typedef typename cplx_of<T>::type C;
+  constexpr int R = 1 << LGR;
+  const int lgLs = lgn - LGR, nb = 1 << lgLs;
+  const int ls = rs * geo_stride(g, lgLs);
+  const bool notw = (lgLs == 0);
+  for (int idx = threadIdx.x; idx < nb * ncol; idx += blockDim.x) {
+    const int i = idx & (nb - 1), cc = idx >> lgLs;
+    C v[R];
+#pragma unroll
+    for (int k = 0; k < R; ++k) v[k] = load(cc, (k << lgLs) + i);
+    dft_reg<LGR, SGN>(v);
+    if (!notw) {
+      const C *twp = tw + g.twoff[0] + i;
+#pragma unroll
+      for (int m = 1; m < R; ++m) {
+        const C w = __ldg(twp + ((m - 1) << lgLs));
+        v[m] = (SGN < 0) ? cmul(v[m], w) : cmulc(v[m], w);
+      }
+    }
+    C *p = buf + (size_t)geo_pad(g, i) * rs + cc;
+#pragma unroll
+    for (int k = 0; k < R; ++k) p[k * ls] = v[k];
+  }
+}
+template <int LGR, int SGN, typename T, typename ST>
+__device__ __forceinline__ void fft_last_to(const Geo &g, const typename cplx_of<T>::type *buf, const typename cplx_of<T>::type *__restrict__ tw,
+                                            int lgn, int ncol, int rs, ST store) {
+  typedef typename cplx_of<T>::type C;
+  constexpr int R = 1 << LGR;
+  const int lgLs = lgn - LGR, nb = 1 << lgLs;
+  const int ls = rs * geo_stride(g, lgLs);
+  const bool notw = (lgLs == 0);
+  for (int idx = threadIdx.x; idx < nb * ncol; idx += blockDim.x) {
+    const int i = idx & (nb - 1), cc = idx >> lgLs;
+    const C *p = buf + (size_t)geo_pad(g, i) * rs + cc;
+    C v[R];
+#pragma unroll
+    for (int k = 0; k < R; ++k) v[k] = p[k * ls];
+    if (!notw) {
+      const C *twp = tw + g.twoff[0] + i;
+#pragma unroll
+      for (int m = 1; m < R; ++m) {
+        const C w = __ldg(twp + ((m - 1) << lgLs));
+        v[m] = (SGN < 0) ? cmul(v[m], w) : cmulc(v[m], w);
+      }
+    }
+    dft_reg<LGR, SGN>(v);
+#pragma unroll
+    for (int k = 0; k < R; ++k) store(cc, (k << lgLs) + i, v[k]);
+  }
+}
+
+/* fft_dif whose input comes from load(cc, j) instead of shared memory.  The caller guarantees that nobody still
+ * reads the buffer; a __syncthreads() is issued after every pass (as fft_dif). */
+template <int SGN, typename T, typename LD>
+__device__ __forceinline__ void fft_dif_from(const Geo &g, typename cplx_of<T>::type *buf, const typename cplx_of<T>::type *__restrict__ tw,
+                                             int ncol, int rs, LD load) {
+  int lgn = 0;
+  for (int q = 0; q < g.nr; ++q) lgn += g.lg[q];
+  switch (g.lg[0]) {
+    case 1: fft_first_from<1, SGN, T>(g, buf, tw, lgn, ncol, rs, load); break;
+    case 2: fft_first_from<2, SGN, T>(g, buf, tw, lgn, ncol, rs, load); break;
+    case 3: fft_first_from<3, SGN, T>(g, buf, tw, lgn, ncol, rs, load); break;
+    default: fft_first_from<4, SGN, T>(g, buf, tw, lgn, ncol, rs, load); break;
+  }
+  __syncthreads();
+  int lgL = lgn - g.lg[0];
+  for (int q = 1; q < g.nr; ++q) {
+    fft_pass_any<SGN, false, T>(g, g.lg[q], buf, tw, lgn, lgL, ncol, rs, g.twoff[q]);
+    lgL -= g.lg[q];
+    __syncthreads();
+  }
+}
+/* fft_dit whose natural-order output goes to store(cc, j, v) instead of shared memory.  Caller guarantees a
+ * __syncthreads() before; NO barrier is issued after the last pass (it only reads the buffer). */
+template <int SGN, typename T, typename ST>
+__device__ __forceinline__ void fft_dit_to(const Geo &g, typename cplx_of<T>::type *buf, const typename cplx_of<T>::type *__restrict__ tw,
+                                           int ncol, int rs, ST store) {
+  int lgn = 0;
+  for (int q = 0; q < g.nr; ++q) lgn += g.lg[q];
+  int lgL = 0;
+  for (int q = g.nr - 1; q >= 1; --q) {
+    lgL += g.lg[q];
+    fft_pass_any<SGN, true, T>(g, g.lg[q], buf, tw, lgn, lgL, ncol, rs, g.twoff[q]);
+    __syncthreads();
+  }
+  switch (g.lg[0]) {
+    case 1: fft_last_to<1, SGN, T>(g, buf, tw, lgn, ncol, rs, store); break;
+    case 2: fft_last_to<2, SGN, T>(g, buf, tw, lgn, ncol, rs, store); break;
+    case 3: fft_last_to<3, SGN, T>(g, buf, tw, lgn, ncol, rs, store); break;
+    default: fft_last_to<4, SGN, T>(g, buf, tw, lgn, ncol, rs, store); break;
+  }
+}
+
 #endif

@@ -98,16 +98,11 @@ __global__ void __launch_bounds__(256, sizeof(T) == 4 ? PSS_MINB : 2) k_update(c
 
   /* ---- phase A: forward FFT of the groups along the last axis ---- */
   if (!A.prologue && P.ngrp > 0) {
-    for (int g = 0; g < P.ngrp; ++g) {
-      const C *src = phat_base + (size_t)g * A.M + (size_t)line0 * n;
-#pragma unroll 4
-      for (int idx = tid; idx < (W << lgn); idx += nt) {
-        const int c = idx >> lgn, j = idx & (n - 1);
-        sm[(size_t)geo_pad(A.geo, j) * RS + g * W + c] = (c < nl) ? src[idx] : zero;
-      }
-    }
-    __syncthreads();
-    fft_dif<-1, T>(A.geo, sm, A.tw, P.ngrp * W, RS);
+    /* the first pass reads the groups straight from global memory (column cc = g*W + c) */
+    fft_dif_from<-1, T>(A.geo, sm, A.tw, P.ngrp * W, RS, [&](int cc, int j) -> C {
+      const int g = cc >> lgW, c = cc & (W - 1);
+      return (c < nl) ? phat_base[(size_t)g * A.M + (size_t)(line0 + c) * n + j] : zero;
+    });
   }
   /* ---- phase B: Eq. 15 + Eq. 16 + Eq. 18 per mode, natural order over k (coalesced state access) ---- */
   for (int c = 0; c < nl; ++c) {
@@ -238,13 +233,11 @@ __global__ void __launch_bounds__(256, sizeof(T) == 4 ? PSS_MINB : 2) k_update(c
       srow[wb * W] = v;
     }
     __syncthreads();
-    fft_dit<+1, T>(A.geo, sm + wb * W, A.tw, W, RS);
+    /* the last pass writes the kept lines straight to global memory (natural order) */
     C *dst = psix_base + (size_t)f * A.M + (size_t)line0 * n;
-#pragma unroll 4
-    for (int idx = tid; idx < (W << lgn); idx += nt) {
-      const int c = idx >> lgn, j = idx & (n - 1);
-      if ((keepmask >> c) & 1u) dst[idx] = sm[(size_t)geo_pad(A.geo, j) * RS + wb * W + c];
-    }
+    fft_dit_to<+1, T>(A.geo, sm + wb * W, A.tw, W, RS, [&](int c, int j, C val) {
+      if ((keepmask >> c) & 1u) dst[(size_t)c * n + j] = val;
+    });
     __syncthreads();
   }
 }
