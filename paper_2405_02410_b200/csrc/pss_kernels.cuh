@@ -243,6 +243,9 @@ __global__ void __launch_bounds__(256, sizeof(T) == 4 ? PSS_MINB : 2) k_update(c
 }
 
 /* ------------------------------------------------------------------------------------------ */
+/* two consecutive rows of one kx: element index kx*R + 2c is even and the arrays are 256-byte aligned */
+template <typename C> struct __align__(16) CPair { C a, b; };
+
 template <typename T> struct RowArgs {
   const typename cplx_of<T>::type *psix; /* [nfac][M]  (kx, r) */
   typename cplx_of<T>::type *phat;       /* [ngrp][M]           */
@@ -279,10 +282,11 @@ __global__ void __launch_bounds__(BIG ? 512 : 256, (!BIG && sizeof(T) == 4) ? PS
       if (cut > nxh) cut = nxh;
     }
     const C *src = psix_base + (size_t)f * A.M + r0;
+#pragma unroll 4
     for (int idx = tid; idx < cut * Wc; idx += nt) {
       const int c = idx & (Wc - 1), kx = idx >> lgWc;
-      const C *p = src + (size_t)kx * A.R + 2 * c;
-      C a = p[0], b = p[1];
+      const CPair<C> pr = *reinterpret_cast<const CPair<C> *>(src + (size_t)kx * A.R + 2 * c); /* rows r, r+1: one 16-byte access (fp32) */
+      C a = pr.a, b = pr.b;
       if (kx == 0 || 2 * kx == nx) { a.y = (T)0; b.y = (T)0; } /* C2R keeps the real part there */
       sm[(size_t)geo_pad(A.geo, kx) * RS + f * Wc + c] = mk<C, T>(a.x - b.y, a.y + b.x);
       if (kx > 0 && 2 * kx < nx) sm[(size_t)geo_pad(A.geo, nx - kx) * RS + f * Wc + c] = mk<C, T>(a.x + b.y, b.x - a.y);
@@ -334,9 +338,10 @@ __global__ void __launch_bounds__(BIG ? 512 : 256, (!BIG && sizeof(T) == 4) ? PS
       const C z = sm[(size_t)geo_pad(A.geo, kx) * RS + wb * Wc + c];
       const C zm = sm[(size_t)geo_pad(A.geo, (nx - kx) & (nx - 1)) * RS + wb * Wc + c];
       const T h = (T)0.5;
-      C *p = dst + (size_t)kx * A.R + 2 * c;
-      p[0] = mk<C, T>(h * (z.x + zm.x), h * (z.y - zm.y));
-      p[1] = mk<C, T>(h * (z.y + zm.y), h * (zm.x - z.x));
+      CPair<C> pr;
+      pr.a = mk<C, T>(h * (z.x + zm.x), h * (z.y - zm.y));
+      pr.b = mk<C, T>(h * (z.y + zm.y), h * (zm.x - z.x));
+      *reinterpret_cast<CPair<C> *>(dst + (size_t)kx * A.R + 2 * c) = pr;
     }
     __syncthreads();
   }
