@@ -313,7 +313,7 @@ def main():
         if tr:
             nsm = torch.cuda.get_device_properties(dev).multi_processor_count
             mhz = (clocks or {}).get("sm_mhz") or 1965.0
-            wi_step = tr["warp_instr_per_launch"] / tr["timesteps_per_launch"]
+            wi_step = R * tr["warp_instr_per_launch"] / tr["timesteps_per_launch"]  # the capture ran one replica
             t_dom = dom_ms * 1e-3 / (prof_n if dom == "k_fused2d" else 1)
             line["roofline"]["issue"] = {"bound": "alu", "unit": "warp-instr/s", "achieved": wi_step / t_dom,
                                          "peak": 4.0 * nsm * mhz * 1e6, "frac": wi_step / t_dom / (4.0 * nsm * mhz * 1e6),
