@@ -300,24 +300,40 @@ int build_program(pss_system *s) {
   if (lin.size() > PSS_P_MAX_LIN) return PSS_EUNSUPPORTED;
   for (size_t i = 0; i < lin.size(); ++i) P.lin[i] = lin[i];
   P.nlin = (int32_t)lin.size();
-  /* radial fast path: all coefficients are polynomials in q^2 */
+  /* radial fast path (pss_program.h): L and the outer operator polynomials in q^2, every factor a polynomial in q^2
+   * times one derivative monomial */
   {
     auto radial = [](const DOp &d) { return d.p == 0 && d.a[0] == 0 && d.a[1] == 0 && d.a[2] == 0 && d.zflags == 0 && d.m <= 4; };
-    bool ok = env_int("PSS_RADIAL", 1) != 0 && P.ndyn == 1 && P.ngrp <= 1 && P.nfac <= 1 &&
-              P.dyn[0].lin_beg == P.dyn[0].lin_end;
+    bool ok = env_int("PSS_RADIAL", 1) != 0 && P.ndyn == 1 && P.ngrp <= 1 && P.dyn[0].lin_beg == P.dyn[0].lin_end;
     if (ok && P.dyn[0].noisy && (P.dyn[0].noise_qpow < 0 || (P.dyn[0].noise_qpow & 1) || P.dyn[0].noise_qpow > 14)) ok = false;
     for (int e = P.dyn[0].lhs_beg; ok && e < P.dyn[0].lhs_end; ++e) ok = radial(P.lin[e]);
     if (ok && P.ngrp == 1) ok = radial(P.grp[0].outer);
-    if (ok && P.nfac == 1)
-      for (int e = P.fac[0].lin_beg; ok && e < P.fac[0].lin_end; ++e) ok = radial(P.lin[e]);
+    for (int f = 0; ok && f < P.nfac; ++f) {
+      const DOp &d0 = P.lin[P.fac[f].lin_beg];
+      for (int e = P.fac[f].lin_beg; ok && e < P.fac[f].lin_end; ++e) {
+        const DOp &d = P.lin[e];
+        ok = d.p == 0 && d.m <= 4 && (d.zflags & 8) == 0 && d.a[0] == d0.a[0] && d.a[1] == d0.a[1] && d.a[2] == d0.a[2] &&
+             d.zflags == d0.zflags && d.a[0] <= 3 && d.a[1] <= 3 && d.a[2] <= 3;
+      }
+      if (P.fac[f].lin_beg == P.fac[f].lin_end) ok = false;
+    }
     if (ok) {
       for (int e = P.dyn[0].lhs_beg; e < P.dyn[0].lhs_end; ++e) P.rad_L[P.lin[e].m] -= P.lin[e].coef;
       if (P.ngrp == 1) P.rad_O[P.grp[0].outer.m] += P.grp[0].outer.coef;
-      if (P.nfac == 1)
-        for (int e = P.fac[0].lin_beg; e < P.fac[0].lin_end; ++e) P.rad_F[P.lin[e].m] += P.lin[e].coef;
+      for (int f = 0; f < P.nfac; ++f) {
+        const DOp &d0 = P.lin[P.fac[f].lin_beg];
+        for (int e = P.fac[f].lin_beg; e < P.fac[f].lin_end; ++e) P.rad_F[f][P.lin[e].m] += P.lin[e].coef;
+        for (int j = 0; j < 3; ++j) P.rad_a[f][j] = d0.a[j];
+        P.rad_a[f][3] = (int8_t)(d0.zflags & 7);
+      }
       P.rad_nhp = P.dyn[0].noisy ? P.dyn[0].noise_qpow / 2 : 0;
     }
-    P.rad_ok = ok ? 1 : 0;
+    P.rad_ok = 0;
+    if (ok) {
+      P.rad_ok = 1; /* 2: some factor carries a derivative monomial */
+      for (int f = 0; f < P.nfac; ++f)
+        if (P.rad_a[f][0] | P.rad_a[f][1] | P.rad_a[f][2]) P.rad_ok = 2;
+    }
   }
   return PSS_OK;
 }
@@ -516,8 +532,9 @@ template <typename T> const typename cplx_of<T>::type *twp(pss_system *s, int ax
 }
 
 template <typename T> int set_attrs(pss_system *s) {
-  CK(cudaFuncSetAttribute(k_update<T, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_MAX));
-  CK(cudaFuncSetAttribute(k_update<T, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_MAX));
+  CK(cudaFuncSetAttribute(k_update<T, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_MAX));
+  CK(cudaFuncSetAttribute(k_update<T, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_MAX));
+  CK(cudaFuncSetAttribute(k_update<T, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_MAX));
   CK(cudaFuncSetAttribute(k_rows<T, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_MAX));
   CK(cudaFuncSetAttribute(k_rows<T, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_MAX));
   CK(cudaFuncSetAttribute(k_mid<-1, T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_MAX));
@@ -643,8 +660,9 @@ template <typename T> int launch_update(pss_system *s, int prologue, uint64_t st
   a.geo = s->plan.geo[s->ndim - 1];
   prof_mark(s, KIND_UPDATE, true);
   const dim3 grid((unsigned)s->plan.upd_blocks, (unsigned)s->nrep);
-  if (P.rad_ok) k_update<T, true><<<grid, s->plan.upd_threads, s->plan.upd_smem, s->stream>>>(P, a);
-  else k_update<T, false><<<grid, s->plan.upd_threads, s->plan.upd_smem, s->stream>>>(P, a);
+  if (P.rad_ok == 1) k_update<T, 1><<<grid, s->plan.upd_threads, s->plan.upd_smem, s->stream>>>(P, a);
+  else if (P.rad_ok == 2) k_update<T, 2><<<grid, s->plan.upd_threads, s->plan.upd_smem, s->stream>>>(P, a);
+  else k_update<T, 0><<<grid, s->plan.upd_threads, s->plan.upd_smem, s->stream>>>(P, a);
   prof_mark(s, KIND_UPDATE, false);
   CKL("k_update");
   if (s->ndim == 3 && P.nfac > 0) return launch_mid<T>(s, +1, s->off_psix, P.nfac, s->plan.kx_keep_max, true, s->nrep);

@@ -73,8 +73,9 @@ template <typename T> __device__ __forceinline__ T horner4(const T (&c)[5], T x)
 }
 
 /* ------------------------------------------------------------------------------------------ */
-/* RAD: the "radial" fast path of pss_program.h (every per-mode coefficient is a polynomial in q^2) */
-template <typename T, bool RAD>
+/* RAD: the "radial" fast path of pss_program.h: 0 = generic term interpreter, 1 = every coefficient a polynomial in
+ * q^2 (Model B, diffusion), 2 = factors carry a derivative monomial on top (KPZ) */
+template <typename T, int RAD>
 __global__ void __launch_bounds__(256, sizeof(T) == 4 ? PSS_MINB : 2) k_update(const __grid_constant__ Program P, const UpdArgs<T> A) {
   typedef typename cplx_of<T>::type C;
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -92,9 +93,9 @@ __global__ void __launch_bounds__(256, sizeof(T) == 4 ? PSS_MINB : 2) k_update(c
   const T qs_last = (T)P.qs[P.ndim - 1];
   const T dt = (T)P.dt, invN = (T)P.invN;
   const C zero = mk<C, T>((T)0, (T)0);
-  T radL[5], radO[5], radF[5];
+  T radL[5], radO[5];
 #pragma unroll
-  for (int i = 0; i < 5; ++i) { radL[i] = (T)P.rad_L[i]; radO[i] = (T)P.rad_O[i]; radF[i] = (T)P.rad_F[i]; }
+  for (int i = 0; i < 5; ++i) { radL[i] = (T)P.rad_L[i]; radO[i] = (T)P.rad_O[i]; }
 
   /* ---- phase A: forward FFT of the groups along the last axis ---- */
   if (!A.prologue && P.ngrp > 0) {
@@ -207,6 +208,11 @@ __global__ void __launch_bounds__(256, sizeof(T) == 4 ? PSS_MINB : 2) k_update(c
       if (kp) keepmask |= 1u << c;
     }
     if (keepmask == 0) continue; /* the whole tile is masked: psix stays zero (zeroed at bind) */
+    T radF[5];
+#pragma unroll
+    for (int i = 0; i < 5; ++i) radF[i] = RAD ? (T)P.rad_F[f][i] : (T)0;
+    const int ra0 = (RAD == 2) ? P.rad_a[f][0] : 0, ra1 = (RAD == 2) ? P.rad_a[f][1] : 0, ra2 = (RAD == 2) ? P.rad_a[f][2] : 0,
+              ra3 = (RAD == 2) ? P.rad_a[f][3] : 0;
     for (int idx = tid; idx < (n << lgW); idx += nt) {
       const int c = idx & (W - 1), s = idx >> lgW;
       C *srow = sm + (size_t)geo_pad(A.geo, s) * RS + c;
@@ -217,9 +223,24 @@ __global__ void __launch_bounds__(256, sizeof(T) == 4 ? PSS_MINB : 2) k_update(c
           const LineQ<T> lq = make_line<T>(P, line0 + c, A.lg_ny);
           const ModeQ<T> mq = line_mode<T>(P, lq, k, n, qs_last);
           if (RAD) {
-            const T fc = horner4<T>(radF, mq.q2) * invN;
+            /* factor f = rad_F[f](q^2) * prod_j (i q_j)^a_j  (pss_program.h) */
+            T fc = horner4<T>(radF, mq.q2) * invN;
             const C ph = srow[0];
-            v = mk<C, T>(ph.x * fc, ph.y * fc);
+            if (RAD == 1) {
+              v = mk<C, T>(ph.x * fc, ph.y * fc);
+            } else {
+              if (ra3 & mq.nyq) fc = (T)0;
+#pragma unroll
+              for (int j = 0; j < 3; ++j) {
+                const int aj = (j == 0) ? ra0 : (j == 1 ? ra1 : ra2);
+                const T qj = mq.q[j];
+                fc *= (aj & 1) ? qj : (T)1;
+                fc *= (aj & 2) ? qj * qj : (T)1;
+              }
+              const int sph = (ra0 + ra1 + ra2) & 3; /* i^s */
+              const T re = ph.x * fc, im = ph.y * fc;
+              v = (sph == 0) ? mk<C, T>(re, im) : (sph == 1) ? mk<C, T>(-im, re) : (sph == 2) ? mk<C, T>(-re, -im) : mk<C, T>(im, -re);
+            }
           } else {
             C phi[PSS_P_MAX_DYN];
 #pragma unroll
@@ -295,7 +316,8 @@ __global__ void __launch_bounds__(BIG ? 512 : 256, (!BIG && sizeof(T) == 4) ? PS
   __syncthreads();
   if (P.nfac > 0) fft_dif<+1, T>(A.geo, sm, A.tw, P.nfac * Wc, RS);
   T pc2 = (T)0, pc3 = (T)0, pc4 = (T)0;
-  if (P.rad_ok && P.ngrp == 1)
+  const bool poly1 = P.rad_ok && P.ngrp == 1 && P.nfac == 1; /* one factor field: the product is a polynomial of it */
+  if (poly1)
     for (int t = P.grp[0].term_beg; t < P.grp[0].term_end; ++t) {
       const T cf = (T)P.term[t].coef;
       if (P.term[t].nf == 2) pc2 += cf;
@@ -311,7 +333,7 @@ __global__ void __launch_bounds__(BIG ? 512 : 256, (!BIG && sizeof(T) == 4) ? PS
       const int sp = geo_pad(A.geo, s);
       const C *srow = sm + (size_t)sp * RS + c;
       T pa = (T)0, pb = (T)0;
-      if (P.rad_ok) {
+      if (poly1) {
         /* one factor field: sum_t coef_t r^nf_t = r^2 (c2 + r (c3 + r c4))  (Eq. 11 with one psi) */
         const C v = srow[0];
         pa = v.x * v.x * (pc2 + v.x * (pc3 + v.x * pc4));

@@ -79,13 +79,18 @@ struct Program {
   DGroup grp[PSS_P_MAX_GRP];
   DTerm term[PSS_P_MAX_TERM];
   DOp lin[PSS_P_MAX_LIN];
-  /* "radial" fast path (set by the host when it applies): one dynamic field, at most one product group and one
-   * factor, no explicit linear terms, every monomial a pure power (q^2)^m with m <= 4, noise power even and >= 0.
-   * Then every per-mode coefficient is a polynomial in q^2 (Horner, ascending coefficients):
-   *   L(q) = rad_L(q^2), outer(q) = rad_O(q^2), factor(q) = rad_F(q^2), noise amp = sqrt(noise_c (q^2)^rad_nhp). */
-  int32_t rad_ok;
+  /* "radial" fast path (set by the host when it applies): one dynamic field, at most one product group, no
+   * explicit linear terms, noise power even and >= 0, and
+   *   L(q) = rad_L(q^2), outer(q) = rad_O(q^2)                     polynomials in q^2 (Horner, ascending, degree <= 4)
+   *   factor f (q) = rad_F[f](q^2) * prod_j (i q_j)^rad_a[f][j]     a polynomial in q^2 times ONE derivative monomial
+   *                                                                  (zero at the Nyquist index of every odd axis, A9)
+   *   noise amp = sqrt(noise_c (q^2)^rad_nhp).
+   * Model B and diffusion have rad_a = 0; KPZ has the factors i q_x h and i q_y h. */
+  int32_t rad_ok; /* 0 no, 1 all rad_a zero, 2 some factor has a derivative monomial */
   int32_t rad_nhp;
-  double rad_L[5], rad_O[5], rad_F[5];
+  double rad_L[5], rad_O[5];
+  double rad_F[PSS_P_MAX_FAC][5];
+  int8_t rad_a[PSS_P_MAX_FAC][4]; /* [3] = zflags & 7 of the monomial */
 };
 
 /* radix schedule of one in-shared-memory FFT of length n = prod R[i] */
