@@ -296,7 +296,8 @@ def main():
                     "h2d_bytes_per_step": len(dyn_names) * S * R, "d2h_bytes_per_step": len(dyn_names) * S * R,
                     "note": "pss_set_field(host) + pss_step(%d) + pss_get_field(host) per bench step" % inner},
             "roofline": {"bound": "hbm", "kernel": dom, "achieved": ach, "peak": peak, "unit": "GB/s",
-                         "frac": ach / peak, "traffic": ncu_traffic(args.workload, dom), "peak_source": peak_src,
+                         "frac": ach / peak, "traffic": (ncu_traffic(args.workload, dom) or {}).get("dram_bytes_per_launch"),
+                         "traffic_capture": ncu_traffic(args.workload, dom), "peak_source": peak_src,
                          "algorithmic_bytes_per_launch": kb[dom], "launch_ms": dom_ms,
                          "timesteps_per_launch": prof_n if dom == "k_fused2d" else 1,
                          "kernel_ms": {k: v[0] for k, v in prof.items() if v[1] > 0},
@@ -309,7 +310,7 @@ def main():
         }
         # secondary reading: the kernels are issue-bound, so also report the issue-slot fraction of the dominant kernel
         # (ncu smsp__inst_executed.sum of the committed capture / its step count, against 4 schedulers x SMs x clock)
-        tr = line["roofline"]["traffic"]
+        tr = line["roofline"]["traffic_capture"]
         if tr:
             nsm = torch.cuda.get_device_properties(dev).multi_processor_count
             mhz = (clocks or {}).get("sm_mhz") or 1965.0

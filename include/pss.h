@@ -104,6 +104,12 @@ int pss_step(pss_system *, int64_t nsteps);
 int pss_get_field(pss_system *, int field, void *real_out, int on_device);
 /* the state in the logical half-spectrum layout, complex of the system precision. */
 int pss_get_field_fourier(pss_system *, int field, void *halfspectrum_out, int on_device);
+/* Checkpoint / resume.  The whole state of a run is the half-spectra of the dynamic fields (pss_get_field_fourier)
+ * plus the step counter, which feeds the noise key.  Restoring both into a freshly built system of the same field
+ * system and seed continues the run bit for bit (the noise is counter-based: SURVEY.md section 5).
+ * halfspectrum_in: logical layout of pss_get_field_fourier, complex of the system precision. */
+int pss_set_field_fourier(pss_system *, int field, const void *halfspectrum_in, int on_device);
+int pss_set_step_count(pss_system *, uint64_t step);
 /* test hook for the noise stream (HOST pointers, either may be NULL): the 4 Philox4x32-10 words per
  * logical mode m, and the unit Hermitian Gaussian z (complex of the system precision) the step uses. */
 int pss_debug_noise(pss_system *, int field, uint64_t step, uint32_t *bits4_per_mode, void *z_halfspectrum);

@@ -20,7 +20,7 @@ OK, EINVAL, EUNSUPPORTED, ESTATE, ECUDA = 0, -1, -2, -3, -4
 
 SYMBOLS = ["pss_create", "pss_add_field", "pss_add_linear", "pss_add_aux_def", "pss_add_term",
            "pss_set_noise", "pss_set_dealias", "pss_set_replicas", "pss_select_replica", "pss_replicas", "pss_finalize", "pss_bind", "pss_set_field", "pss_step",
-           "pss_get_field", "pss_get_field_fourier", "pss_debug_noise", "pss_profile_step", "pss_uses_fused_kernel", "pss_launch_count",
+           "pss_get_field", "pss_get_field_fourier", "pss_set_field_fourier", "pss_set_step_count", "pss_debug_noise", "pss_profile_step", "pss_uses_fused_kernel", "pss_launch_count",
            "pss_model_bytes_per_step", "pss_step_count", "pss_strerror", "pss_last_cuda_error",
            "pss_destroy"]
 
@@ -69,6 +69,8 @@ def lib():
         L.pss_step.argtypes = [P, C.c_int64]
         L.pss_get_field.argtypes = [P, C.c_int, P, C.c_int]
         L.pss_get_field_fourier.argtypes = [P, C.c_int, P, C.c_int]
+        L.pss_set_field_fourier.argtypes = [P, C.c_int, P, C.c_int]
+        L.pss_set_step_count.argtypes = [P, C.c_uint64]
         L.pss_debug_noise.argtypes = [P, C.c_int, C.c_uint64, P, P]
         L.pss_profile_step.argtypes = [P, C.c_int64, C.POINTER(C.c_double), C.POINTER(C.c_int64)]
         L.pss_uses_fused_kernel.argtypes = [P]
@@ -223,6 +225,15 @@ class System:
         out = np.empty(self.hshape, dtype=self.cdtype)
         self._chk(lib().pss_get_field_fourier(self._h, int(field), out.ctypes.data_as(C.c_void_p), 0))
         return out
+
+    def set_field_fourier(self, field, spec):
+        """restore a half-spectrum written by get_field_fourier (numpy complex array, logical layout)"""
+        a = np.ascontiguousarray(np.asarray(spec), dtype=self.cdtype)
+        assert a.shape == tuple(self.hshape), (a.shape, self.hshape)
+        self._chk(lib().pss_set_field_fourier(self._h, int(field), a.ctypes.data_as(C.c_void_p), 0))
+
+    def set_step_count(self, step):
+        self._chk(lib().pss_set_step_count(self._h, C.c_uint64(int(step))))
 
     def debug_noise(self, field, step):
         nm = int(np.prod(self.hshape))

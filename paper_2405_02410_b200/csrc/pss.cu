@@ -851,6 +851,20 @@ template <typename T> int do_get_fourier(pss_system *s, int slot, void *dst, int
   return PSS_OK;
 }
 
+template <typename T> int do_set_fourier(pss_system *s, int slot, const void *src, int on_device) {
+  typedef typename cplx_of<T>::type C;
+  const C *in = (const C *)src;
+  if (!on_device) {
+    CK(cudaMemcpyAsync(s->ws + s->off_scratch, src, (size_t)s->M * sizeof(C), cudaMemcpyHostToDevice, s->stream));
+    in = carr<T>(s, s->off_scratch, 0);
+  }
+  k_from_logical<T><<<592, 256, 0, s->stream>>>(in, carr<T>(s, s->off_state, s->sel * s->P.ndyn + slot), s->P.nxh, (int)s->n[1], (int)s->n[2]);
+  CKL("k_from_logical");
+  s->psix_valid = false;
+  if (!on_device) CK(cudaStreamSynchronize(s->stream));
+  return PSS_OK;
+}
+
 template <typename T> int do_debug_noise(pss_system *s, int field, uint64_t step, uint32_t *bits, void *z) {
   typedef typename cplx_of<T>::type C;
   uint32_t *dbits = nullptr;
@@ -1068,6 +1082,21 @@ int pss_get_field_fourier(pss_system *s, int field, void *out, int on_device) {
   const int slot = s->dyn_slot[field];
   return (s->prec == PSS_F32) ? do_get_fourier<float>(s, slot, out, on_device)
                               : do_get_fourier<double>(s, slot, out, on_device);
+}
+
+int pss_set_field_fourier(pss_system *s, int field, const void *in, int on_device) {
+  if (!s || !in) return PSS_EINVAL;
+  if (!s->finalized || !s->bound) return PSS_ESTATE;
+  if (s->cuda_bad) return PSS_ECUDA;
+  if (!fid_ok(s, field) || !s->fields[field].dynamic) return PSS_EINVAL;
+  const int slot = s->dyn_slot[field];
+  return (s->prec == PSS_F32) ? do_set_fourier<float>(s, slot, in, on_device) : do_set_fourier<double>(s, slot, in, on_device);
+}
+
+int pss_set_step_count(pss_system *s, uint64_t step) {
+  if (!s) return PSS_EINVAL;
+  s->step = step;
+  return PSS_OK;
 }
 
 int pss_debug_noise(pss_system *s, int field, uint64_t step, uint32_t *bits, void *z) {

@@ -492,6 +492,18 @@ __global__ void k_to_logical(const typename cplx_of<T>::type *arr, typename cplx
   }
 }
 
+/* logical [r'][kx] -> internal [kx][r] for pss_set_field_fourier (checkpoint restore) */
+template <typename T>
+__global__ void k_from_logical(const typename cplx_of<T>::type *in, typename cplx_of<T>::type *arr, int nxh, int ny, int nz) {
+  const long long total = (long long)nxh * ny * nz;
+  for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < total; i += (long long)gridDim.x * blockDim.x) {
+    const int kx = (int)(i % nxh);
+    const long long rp = i / nxh;
+    const long long y = rp % ny, z = rp / ny;
+    arr[(size_t)kx * ny * nz + y * nz + z] = in[i];
+  }
+}
+
 /* noise test hook: Philox words and z per logical mode */
 template <typename T>
 __global__ void k_debug_noise(const __grid_constant__ Program P, unsigned rep, int field, unsigned long long step, uint32_t *bits,
