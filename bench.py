@@ -55,7 +55,7 @@ class ClockSampler:
         self.proc = None
         try:
             self.proc = subprocess.Popen(["nvidia-smi", "-i", str(index), "--query-gpu=" + self.Q,
-                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                          "--format=csv,noheader,nounits", "-lms", "25"],
                                          stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.t = threading.Thread(target=self._read, daemon=True)
             self.t.start()
@@ -109,19 +109,28 @@ def oracle_rate(cfg, prec, budget_s, max_steps):
 
 
 def run_reference(args, cfg, rank, world):
+    """--impl reference: the CPU oracle as it stands on the host cores, same workload/metric/unit.  One bench step is
+    a bounded sample of oracle time steps (ref_budget / steps seconds, at least one time step)."""
     if rank != 0:
         return
-    per = []
-    for _ in range(args.warmup):
-        pass  # the oracle has no warm state beyond its own first step (done inside oracle_rate)
+    from oracle import opss
+    o, _ = wl.build(opss, cfg, prec=args.prec)
+    for _ in range(max(1, args.warmup)):
+        o.step(1)
     sites = int(np.prod(cfg["n"]))
+    per_step_budget = args.ref_budget / max(1, args.steps)
     total_steps, total_t = 0, 0.0
-    cores = 1
     for _ in range(args.steps):
-        r, n, el, cores = oracle_rate(cfg, args.prec, args.ref_budget / max(1, args.steps), 64)
-        per.append(r)
+        n, t0 = 0, time.perf_counter()
+        while True:
+            o.step(1)
+            n += 1
+            el = time.perf_counter() - t0
+            if el >= per_step_budget:
+                break
         total_steps += n
         total_t += el
+    cores = int(os.environ.get("OMP_NUM_THREADS", "0")) or (os.cpu_count() or 1)
     v = total_steps / total_t
     line = {
         "impl": "reference", "metric": "timesteps/s", "value": v, "unit": "timesteps/s", "n_gpus": args.gpus,
@@ -129,7 +138,7 @@ def run_reference(args, cfg, rank, world):
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "site_updates_per_s": v * sites,
         "config": {"workload": args.workload, "lattice": list(cfg["n"]), "precision": args.prec,
-                   "note": "CPU oracle (oracle/opss.cpp) as it stands; each step is a bounded sample of oracle time steps"},
+                   "note": "CPU oracle (oracle/opss.cpp) as it stands; each bench step is a bounded sample of oracle time steps"},
         "cpu_baseline": {"value": v, "unit": "timesteps/s", "cores": cores, "kind": "oracle",
                          "sample": "%d oracle time steps of %s in %.1f s" % (total_steps, args.workload, total_t)},
         "e2e": {"value": v, "unit": "timesteps/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
@@ -141,7 +150,7 @@ def run_reference(args, cfg, rank, world):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--steps", type=int, default=100)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--inner", type=int, default=500, help="time steps per bench step (one pss_step call)")
     ap.add_argument("--workload", default="modelb_1024")
@@ -204,6 +213,8 @@ def main():
     reseed = cfg["model"] == "nematic"
     inner = min(args.inner, 250) if reseed else args.inner
 
+    # clocks / throttle reasons are sampled from before the warm-up (same kernels, same load) to the end of the timed region
+    sampler = ClockSampler(local_rank) if rank == 0 else None
     for _ in range(max(args.warmup, 0)):
         if reseed:
             reset_state()
@@ -211,7 +222,6 @@ def main():
     barrier()
 
     launches0 = g.launch_count
-    sampler = ClockSampler(local_rank) if rank == 0 else None
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
     barrier()
     launches_timed = 0
@@ -320,7 +330,7 @@ def main():
                                          "peak": 4.0 * nsm * mhz * 1e6, "frac": wi_step / t_dom / (4.0 * nsm * mhz * 1e6),
                                          "note": "instruction-issue slots: 4 schedulers per SM x 1 warp-instr per clock"}
         if not args.no_cpu_baseline and world == 1:
-            r, n, el, cores = oracle_rate(cfg, args.prec, args.cpu_budget, 64)
+            r, n, el, cores = oracle_rate(cfg, args.prec, args.cpu_budget, 10 ** 6)
             line["cpu_baseline"] = {"value": r, "unit": "timesteps/s", "cores": cores, "kind": "oracle",
                                     "sample": "%d oracle time steps of %s after 1 warm-up step, %.1f s" % (n, args.workload, el)}
         if not args.no_compare and world == 1 and cfg["model"] == "model_b" and len(cfg["n"]) == 2 and args.prec == "f32":
