@@ -300,6 +300,9 @@ int build_program(pss_system *s) {
   if (lin.size() > PSS_P_MAX_LIN) return PSS_EUNSUPPORTED;
   for (size_t i = 0; i < lin.size(); ++i) P.lin[i] = lin[i];
   P.nlin = (int32_t)lin.size();
+  P.any_invq = 0;
+  for (const DOp &d : lin) if (d.p > 0) P.any_invq = 1;
+  for (int g = 0; g < P.ngrp; ++g) if (P.grp[g].outer.p > 0) P.any_invq = 1;
   /* radial fast path (pss_program.h): L and the outer operator polynomials in q^2, every factor a polynomial in q^2
    * times one derivative monomial */
   {

@@ -66,6 +66,7 @@ template <typename T> __device__ __forceinline__ ModeQ<T> line_mode(const Progra
   if (P.ndim == 3) { mq.q[1] = l.q1; mq.q[2] = ql; mq.nyq = l.nyq | (last_nyq << 2); }
   else { mq.q[1] = ql; mq.q[2] = (T)0; mq.nyq = l.nyq | (last_nyq << 1); }
   mq.q2 = l.q2line + ql * ql;
+  mq.rq = (P.any_invq && mq.q2 > (T)0) ? (T)1 / sqrt(mq.q2) : (T)0;
   return mq;
 }
 template <typename T> __device__ __forceinline__ T horner4(const T (&c)[5], T x) {

@@ -12,6 +12,7 @@
 template <typename T> struct ModeQ {
   T q[3];
   T q2;
+  T rq;    /* 1/|q| (0 at q = 0, A10); filled only when the program has a 1/q keyword (Program::any_invq) */
   int nyq; /* bit j set: k_j is the Nyquist index of axis j */
 };
 
@@ -32,6 +33,7 @@ template <typename T> __device__ __forceinline__ ModeQ<T> make_mode(const Progra
     }
     mq.q2 += mq.q[j] * mq.q[j];
   }
+  mq.rq = (P.any_invq && mq.q2 > (T)0) ? (T)1 / sqrt(mq.q2) : (T)0;
   return mq;
 }
 
@@ -45,7 +47,7 @@ template <typename T> __device__ __forceinline__ typename cplx_of<T>::type eval_
     for (int m = op.m; m > 0; m >>= 1) { if (m & 1) r *= bq; bq *= bq; }
   }
   if (op.p > 0) {
-    T bq = (T)1 / sqrt(mq.q2);
+    T bq = mq.rq;
     for (int m = op.p; m > 0; m >>= 1) { if (m & 1) r *= bq; bq *= bq; }
   }
   int s = 0;

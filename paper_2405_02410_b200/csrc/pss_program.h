@@ -73,7 +73,7 @@ struct Program {
   double invN;
   uint32_t seed_lo, seed_hi;
   int32_t ndyn, nfac, ngrp, nterm, nlin;
-  int32_t pad_;
+  int32_t any_invq; /* some monomial uses the 1/q keyword: the kernels then evaluate 1/|q| once per mode */
   DDyn dyn[PSS_P_MAX_DYN];
   DFactor fac[PSS_P_MAX_FAC];
   DGroup grp[PSS_P_MAX_GRP];
