@@ -186,7 +186,12 @@ __device__ __forceinline__ void grid_barrier(unsigned long long *ctr, unsigned l
   if ((threadIdx.x & (TT - 1)) == 0) {
     asm volatile("red.release.gpu.global.add.u64 [%0], 1;" ::"l"(ctr) : "memory");
     unsigned long long v;
-    do { asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(ctr) : "memory"); } while (v < target);
+    unsigned spins = 0;
+    for (;;) {
+      asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(ctr) : "memory");
+      if (v >= target) break;
+      if (++spins > (1u << 25)) __trap(); /* watchdog (tens of seconds): fail the launch instead of hanging the GPU */
+    }
   }
   tsync();
 }
