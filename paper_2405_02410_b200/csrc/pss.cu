@@ -451,7 +451,7 @@ int make_plan(pss_system *s) {
     if (per > SMEM_MAX) return PSS_EUNSUPPORTED;
     int W = 1;
     for (int cand = 8; cand >= 1; cand >>= 1) {
-      if (per * cand > SMEM_SOFT && cand > 1) continue;
+      if (per * cand > 40 * 1024 && cand > 1) continue; /* measured: small tiles win once a line fills ~32 KB */
       if ((nlines + cand - 1) / cand < 2 * 148 && cand > 1) continue;
       W = cand;
       break;
@@ -463,7 +463,10 @@ int make_plan(pss_system *s) {
     pl.upd_W = W;
     pl.upd_smem = per * W;
     pl.upd_blocks = (int)((nlines + W - 1) / W);
-    pl.upd_threads = env_int("PSS_UPD_T", round_threads((n / 8) * W * (P.ngrp > 0 ? P.ngrp : 1)));
+    pl.upd_threads = round_threads((n / 8) * W * (P.ngrp > 0 ? P.ngrp : 1));
+    /* short lines in a big grid (3D): one thread per radix-16 butterfly and more, smaller CTAs per SM (measured) */
+    if ((n / 16) * W * (P.ngrp > 0 ? P.ngrp : 1) <= 128 && pl.upd_blocks >= 12 * 148 && pl.upd_threads > 128) pl.upd_threads = 128;
+    pl.upd_threads = env_int("PSS_UPD_T", pl.upd_threads);
   }
   /* k_rows: Wc pairs of rows per CTA (2*Wc contiguous rows of every kx) */
   if (P.ngrp > 0) {
@@ -489,6 +492,7 @@ int make_plan(pss_system *s) {
     pl.row_smem = per * Wc;
     pl.row_blocks = (int)(R / (2 * Wc));
     pl.row_threads = round_threads((nx / 8) * Wc * (P.nfac > 0 ? P.nfac : 1));
+    if ((nx / 16) * Wc * (P.nfac > 0 ? P.nfac : 1) <= 128 && pl.row_blocks >= 12 * 148 && pl.row_threads > 128) pl.row_threads = 128;
     /* a tile that leaves room for one CTA per SM only gets 512 threads (fp32; the fp64 butterflies need the registers) */
     if (pl.row_smem > 113 * 1024 && cs == 8 && (nx / 16) * Wc * (P.nfac > 0 ? P.nfac : 1) >= 512) pl.row_threads = 512;
     pl.row_threads = env_int("PSS_ROW_T", pl.row_threads);
