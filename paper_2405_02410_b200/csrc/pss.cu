@@ -499,13 +499,13 @@ int make_plan(pss_system *s) {
     if (pl.row_threads > 512) pl.row_threads = 512;
   }
   if (s->ndim == 3) {
-    int W = (int)(128 / cs);
+    int W = env_int("PSS_MID_W", (int)(128 / cs));
     if (W > s->n[2]) W = (int)s->n[2];
     while ((size_t)W * pl.geo[1].npad * cs > SMEM_MAX && W > 1) W >>= 1;
     if ((size_t)W * pl.geo[1].npad * cs > SMEM_MAX) return PSS_EUNSUPPORTED;
     pl.mid_W = W;
     pl.mid_smem = (size_t)W * pl.geo[1].npad * cs;
-    pl.mid_threads = round_threads((s->n[1] / 8) * W);
+    pl.mid_threads = env_int("PSS_MID_T", round_threads((s->n[1] / 32) * W)); /* two radix-16 butterflies per thread (measured) */
   }
   return PSS_OK;
 }
