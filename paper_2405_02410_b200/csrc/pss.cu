@@ -466,6 +466,8 @@ int make_plan(pss_system *s) {
     pl.upd_threads = round_threads((n / 8) * W * (P.ngrp > 0 ? P.ngrp : 1));
     /* short lines in a big grid (3D): one thread per radix-16 butterfly and more, smaller CTAs per SM (measured) */
     if ((n / 16) * W * (P.ngrp > 0 ? P.ngrp : 1) <= 128 && pl.upd_blocks >= 12 * 148 && pl.upd_threads > 128) pl.upd_threads = 128;
+    /* small lattices are latency-bound: at least n/2 threads (128..256) for the pointwise stage (measured) */
+    if (n <= 512 && pl.upd_threads < 128) pl.upd_threads = (n >= 512) ? 256 : 128;
     pl.upd_threads = env_int("PSS_UPD_T", pl.upd_threads);
   }
   /* k_rows: Wc pairs of rows per CTA (2*Wc contiguous rows of every kx) */
