@@ -41,6 +41,7 @@ struct Plan {
   int kx_keep_max;                  /* max over factors of the number of kept kx */
   int fused;                        /* 1: the persistent 1024^2 fp32 kernel of pss_fused2d.cuh runs the steps (PSS_FUSED=0 disables) */
   int fused_prune;                  /* its input-pruned instantiation (mask cutoff <= n/4 on both axes)       */
+  int pdl;                          /* programmatic dependent launch between the step kernels (PSS_PDL=0 disables) */
   int fused_pair;                   /* ensembles: two replicas per launch (k_fused2d_pair)                    */
 };
 
@@ -429,6 +430,7 @@ int make_plan(pss_system *s) {
     }
     if (cut > pl.kx_keep_max) pl.kx_keep_max = cut;
   }
+  pl.pdl = env_int("PSS_PDL", 1);
   pl.fused = fused2d_eligible(s) ? 1 : 0;
   if (pl.fused) {
     const int nn = (P.dealias == PSS_DEALIAS_OFF) ? 1 : ((P.dealias == PSS_DEALIAS_TWO_THIRDS ? 2 : P.fac[0].order) + 1);
@@ -626,6 +628,24 @@ void prof_mark(pss_system *s, int kind, bool begin) {
   if (begin) s->prof_kind.push_back(kind);
 }
 
+/* Programmatic dependent launch: the next kernel of the step is launched while the previous one drains; every step
+ * kernel starts with griddepcontrol.wait, so nothing is read or written before the previous grid has completed. */
+template <typename... KArgs, typename... Args>
+cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, unsigned threads, size_t smem, cudaStream_t stream, bool pdl, Args... args) {
+  cudaLaunchConfig_t cfg;
+  std::memset(&cfg, 0, sizeof(cfg));
+  cfg.gridDim = grid;
+  cfg.blockDim = dim3(threads);
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = stream;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = at;
+  cfg.numAttrs = pdl ? 1 : 0;
+  return cudaLaunchKernelEx(&cfg, kernel, args...);
+}
+
 template <typename T> int launch_mid(pss_system *s, int sgn, size_t off, int nbatch, int kx_count, bool factor_mask = false, int nrep = 1) {
   MidArgs<T> a;
   std::memset(&a, 0, sizeof(a));
@@ -669,9 +689,10 @@ template <typename T> int launch_update(pss_system *s, int prologue, uint64_t st
   a.geo = s->plan.geo[s->ndim - 1];
   prof_mark(s, KIND_UPDATE, true);
   const dim3 grid((unsigned)s->plan.upd_blocks, (unsigned)s->nrep);
-  if (P.rad_ok == 1) k_update<T, 1><<<grid, s->plan.upd_threads, s->plan.upd_smem, s->stream>>>(P, a);
-  else if (P.rad_ok == 2) k_update<T, 2><<<grid, s->plan.upd_threads, s->plan.upd_smem, s->stream>>>(P, a);
-  else k_update<T, 0><<<grid, s->plan.upd_threads, s->plan.upd_smem, s->stream>>>(P, a);
+  const bool pdl = s->plan.pdl != 0;
+  if (P.rad_ok == 1) launch_pdl(k_update<T, 1>, grid, s->plan.upd_threads, s->plan.upd_smem, s->stream, pdl, P, a);
+  else if (P.rad_ok == 2) launch_pdl(k_update<T, 2>, grid, s->plan.upd_threads, s->plan.upd_smem, s->stream, pdl, P, a);
+  else launch_pdl(k_update<T, 0>, grid, s->plan.upd_threads, s->plan.upd_smem, s->stream, pdl, P, a);
   prof_mark(s, KIND_UPDATE, false);
   CKL("k_update");
   if (s->ndim == 3 && P.nfac > 0) return launch_mid<T>(s, +1, s->off_psix, P.nfac, s->plan.kx_keep_max, true, s->nrep);
@@ -691,8 +712,9 @@ template <typename T> int launch_rows(pss_system *s) {
   a.geo = s->plan.geo[0];
   prof_mark(s, KIND_ROWS, true);
   const dim3 grid((unsigned)s->plan.row_blocks, (unsigned)s->nrep);
-  if (s->plan.row_threads > 256) k_rows<T, true><<<grid, s->plan.row_threads, s->plan.row_smem, s->stream>>>(P, a);
-  else k_rows<T, false><<<grid, s->plan.row_threads, s->plan.row_smem, s->stream>>>(P, a);
+  const bool pdl = s->plan.pdl != 0;
+  if (s->plan.row_threads > 256) launch_pdl(k_rows<T, true>, grid, s->plan.row_threads, s->plan.row_smem, s->stream, pdl, P, a);
+  else launch_pdl(k_rows<T, false>, grid, s->plan.row_threads, s->plan.row_smem, s->stream, pdl, P, a);
   prof_mark(s, KIND_ROWS, false);
   CKL("k_rows");
   if (s->ndim == 3) return launch_mid<T>(s, -1, s->off_phat, P.ngrp, P.nxh, false, s->nrep);

@@ -19,6 +19,11 @@
 #define PSS_KERNELS_CUH
 #include "pss_pointwise.cuh"
 
+/* programmatic dependent launch: block until the previous kernel of the stream has completed and its writes are
+ * visible (a no-op when the launch carries no such dependency) */
+/* (an early griddepcontrol.launch_dependents was measured slower and is not used) */
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+
 #ifndef PSS_MINB
 #define PSS_MINB 3 /* fp32 k_rows / k_update: resident CTAs per SM the register budget is tuned for */
 #endif
@@ -81,6 +86,7 @@ __global__ void __launch_bounds__(256, sizeof(T) == 4 ? PSS_MINB : 2) k_update(c
   typedef typename cplx_of<T>::type C;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   C *sm = reinterpret_cast<C *>(smem_raw);
+  pdl_wait();
   const int n = A.n, W = A.W, lgn = A.lgn, lgW = A.lgW;
   const int line0 = blockIdx.x * W;
   const unsigned rep = blockIdx.y; /* ensemble replica: arrays [replica][field][M] */
@@ -285,6 +291,7 @@ __global__ void __launch_bounds__(BIG ? 512 : 256, (!BIG && sizeof(T) == 4) ? PS
   typedef typename cplx_of<T>::type C;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   C *sm = reinterpret_cast<C *>(smem_raw);
+  pdl_wait();
   const int nx = A.nx, nxh = nx / 2 + 1, Wc = A.Wc, lgWc = 31 - __clz(Wc); /* Wc is a power of two */
   const int RS = (P.nfac + (P.ngrp > 1 ? 1 : 0)) * Wc;
   const long long r0 = (long long)blockIdx.x * (2 * Wc);
