@@ -663,8 +663,8 @@ template <typename T> int launch_mid(pss_system *s, int sgn, size_t off, int nba
   a.geo = s->plan.geo[1];
   dim3 grid((unsigned)(s->n[2] / s->plan.mid_W), (unsigned)kx_count, (unsigned)(nbatch * nrep));
   prof_mark(s, KIND_MID, true);
-  if (sgn < 0) k_mid<-1, T><<<grid, s->plan.mid_threads, s->plan.mid_smem, s->stream>>>(a);
-  else k_mid<+1, T><<<grid, s->plan.mid_threads, s->plan.mid_smem, s->stream>>>(a);
+  if (sgn < 0) launch_pdl(k_mid<-1, T>, grid, s->plan.mid_threads, s->plan.mid_smem, s->stream, s->plan.pdl != 0, a);
+  else launch_pdl(k_mid<+1, T>, grid, s->plan.mid_threads, s->plan.mid_smem, s->stream, s->plan.pdl != 0, a);
   prof_mark(s, KIND_MID, false);
   CKL("k_mid");
   return PSS_OK;

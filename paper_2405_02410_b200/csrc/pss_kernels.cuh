@@ -396,6 +396,7 @@ template <int SGN, typename T> __global__ void __launch_bounds__(256) k_mid(cons
   typedef typename cplx_of<T>::type C;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   C *sm = reinterpret_cast<C *>(smem_raw);
+  pdl_wait();
   const int W = A.W, ny = A.ny;
   const int kx = blockIdx.y;
   if (kx >= A.kx_count) return;
