@@ -12,6 +12,7 @@
 #include <cuda_runtime.h>
 #include <cufft.h>
 #include <curand.h>
+#include <curand_kernel.h>
 #include <math.h>
 #include <stdint.h>
 
@@ -102,4 +103,28 @@ extern "C" int cmp_cufft_modelb(int nx, int ny, double dx, double dt, double a, 
   if (r2c) cufftDestroy(r2c);
   cudaFree(phi); cudaFree(psi); cudaFree(eta); cudaFree(real); cudaFree(white);
   return rc;
+}
+
+/* Pin P8: the Philox4x32-10 block of cuRAND's DEVICE API for (seed, subsequence, offset): with
+ * curand_init(seed, subsequence, offset) the key is the seed, (c2, c3) = subsequence and (c0, c1) = offset / 4, so
+ * the block (c0, c1, c2, c3) is subsequence = c2 | c3 << 32, offset = 4 (c0 | c1 << 32) followed by one curand4().
+ * Test infrastructure for tests/ only (an independent implementation to compare the oracle's and the product's
+ * Philox against); the product never calls it. */
+namespace {
+__global__ void k_curand_block(unsigned long long seed, unsigned long long subsequence, unsigned long long offset, unsigned int *out) {
+  curandStatePhilox4_32_10_t st;
+  curand_init(seed, subsequence, offset, &st);
+  const uint4 r = curand4(&st);
+  out[0] = r.x; out[1] = r.y; out[2] = r.z; out[3] = r.w;
+}
+}  // namespace
+
+extern "C" int cmp_curand_philox_block(unsigned long long seed, unsigned long long subsequence, unsigned long long offset,
+                                       unsigned int out4[4]) {
+  unsigned int *d = nullptr;
+  if (cudaMalloc(&d, 4 * sizeof(unsigned int)) != cudaSuccess) return -1;
+  k_curand_block<<<1, 1>>>(seed, subsequence, offset, d);
+  const cudaError_t e = cudaMemcpy(out4, d, 4 * sizeof(unsigned int), cudaMemcpyDeviceToHost);
+  cudaFree(d);
+  return e == cudaSuccess ? 0 : -1;
 }

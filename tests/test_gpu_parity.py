@@ -205,3 +205,34 @@ def test_error_codes_on_gpu(pss):
     with pytest.raises(b.PssError) as e:
         s.step(1)
     assert e.value.code == b.ESTATE
+
+
+def test_p8_philox_matches_curand_device_api(pss, oracle):
+    """P8: the oracle's Philox4x32-10 block and the words the CUDA path draws equal cuRAND's device
+    generator (curand_init + curand4) for the same key and counter — an implementation neither side wrote."""
+    import ctypes
+    from paper_2405_02410_b200 import build
+    lib = ctypes.CDLL(build.build_compare())
+    lib.cmp_curand_philox_block.argtypes = [ctypes.c_uint64, ctypes.c_uint64, ctypes.c_uint64, ctypes.POINTER(ctypes.c_uint32)]
+
+    def curand_block(ctr, key):
+        out = (ctypes.c_uint32 * 4)()
+        rc = lib.cmp_curand_philox_block(key[0] | (key[1] << 32), ctr[2] | (ctr[3] << 32), 4 * (ctr[0] | (ctr[1] << 32)), out)
+        assert rc == 0
+        return tuple(int(v) for v in out)
+
+    rng = np.random.default_rng(11)
+    cases = [((0, 0, 0, 0), (0, 0)), ((1, 0, 0, 0), (0, 0)), ((0, 0, 1, 0), (0, 0))]
+    for _ in range(12):   # offset = 4 * (c0 | c1 << 32) must fit 64 bits: c1 < 2^30
+        cases.append(((int(rng.integers(0, 2 ** 32)), int(rng.integers(0, 2 ** 30)), int(rng.integers(0, 2 ** 32)),
+                       int(rng.integers(0, 2 ** 32))), tuple(int(v) for v in rng.integers(0, 2 ** 32, 2))))
+    for ctr, key in cases:
+        assert oracle.philox(ctr, key) == curand_block(ctr, key), (ctr, key)
+    # and the words the product draws for (seed, step, field, mode) are that block
+    cfg = wl.make_config("modelb_128", n=(16, 8))
+    g, ids = wl.build(pss, cfg, prec="f32")
+    bits, _ = g.debug_noise(ids["phi"], 7)
+    seed = cfg["seed"]
+    for (ky, kx) in [(0, 0), (5, 3), (7, 8)]:
+        m = ky * 9 + kx
+        assert tuple(int(v) for v in bits[ky, kx]) == curand_block((m, 0, 7, ids["phi"]), (seed & 0xffffffff, seed >> 32))
