@@ -108,6 +108,16 @@ def oracle_rate(cfg, prec, budget_s, max_steps):
     return n / el, n, el, cores
 
 
+def bench_config(args, cfg, R):
+    """the `config` object of the JSON line: the workload, identical for the CUDA arm and the reference arm"""
+    return {"workload": args.workload, "lattice": list(cfg["n"]), "precision": args.prec,
+            "timesteps_per_bench_step": int(min(args.inner, 250) if cfg["model"] == "nematic" else args.inner),
+            "replicas_per_gpu": int(R),
+            "parallelism": "replicas only (independent realisations; value counts replica time steps)",
+            "l2": "flushed between timed bench steps (256 MiB written); inside a bench step the "
+                  "time stepper reuses its own state, as the workload does"}
+
+
 def run_reference(args, cfg, rank, world):
     """--impl reference: the CPU oracle as it stands on the host cores, same workload/metric/unit.  One bench step is
     a bounded sample of oracle time steps (ref_budget / steps seconds, at least one time step)."""
@@ -137,8 +147,9 @@ def run_reference(args, cfg, rank, world):
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * total_t / max(1, args.steps),
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "site_updates_per_s": v * sites,
-        "config": {"workload": args.workload, "lattice": list(cfg["n"]), "precision": args.prec,
-                   "note": "CPU oracle (oracle/opss.cpp) as it stands; each bench step is a bounded sample of oracle time steps"},
+        "config": bench_config(args, cfg, 1),
+        "note": "CPU oracle (oracle/opss.cpp) as it stands; each bench step is a bounded sample of oracle time steps "
+                "of the workload that config names",
         "cpu_baseline": {"value": v, "unit": "timesteps/s", "cores": cores, "kind": "oracle",
                          "sample": "%d oracle time steps of %s in %.1f s" % (total_steps, args.workload, total_t)},
         "e2e": {"value": v, "unit": "timesteps/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
@@ -294,12 +305,8 @@ def main():
             "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": args.prec, "data": "synthetic",
             "site_updates_per_s": value * sites, "us_per_timestep": step_ms * 1e3, "us_per_replica_timestep": step_ms * 1e3 / R,
-            "config": {"workload": args.workload, "lattice": list(cfg["n"]), "precision": args.prec,
-                       "timesteps_per_bench_step": inner, "replicas_per_gpu": R,
-                       "parallelism": "replicas only (independent realisations; value counts replica time steps)",
-                       "l2": "flushed between timed bench steps (256 MiB written); inside a bench step the "
-                             "time stepper reuses its own state, as the workload does",
-                       "final_state_finite": finite},
+            "config": bench_config(args, cfg, R),
+            "final_state_finite": finite,
             "gpu_launches": int(launches_timed),
             "clocks": clocks,
             "e2e": {"value": e2e_value, "unit": "timesteps/s",
@@ -342,12 +349,12 @@ def main():
 
 def cufft_compare(cfg):
     """The same 2D Model-B step built the way the paper describes its GPU path (cuFFT for every transform, cuRAND
-    noise, one pointwise kernel per arrow; paper_2405_02410_b200/compare/cufft_modelb.cu), timed with CUDA events on
+    noise, one pointwise kernel per arrow; compare/cufft_modelb.cu), timed with CUDA events on
     this GPU.  A comparison baseline only (north_star); the product never loads it."""
     import ctypes
     try:
-        from paper_2405_02410_b200 import build as pss_build
-        lib = ctypes.CDLL(pss_build.build_compare())
+        from compare import build as compare_build
+        lib = ctypes.CDLL(compare_build.build())
         us = ctypes.c_double(0.0)
         pr = cfg["params"]
         nsteps = 200 if cfg["n"][0] <= 2048 else 30

@@ -84,7 +84,8 @@ int pss_set_dealias(pss_system *, int rule);
 /* Ensemble (stochastic studies need many realisations): the system holds
  * `nreplicas` independent realisations of the same field system and pss_step advances all of them in the same
  * launches (grid dimension y).  Replica r is, bit for bit, the system created with seed + r.  Call before
- * pss_finalize; 1 <= nreplicas <= 65535.  The persistent 1024^2 kernel runs the replicas one launch after the other. */
+ * pss_finalize; 1 <= nreplicas <= 65535, and in 3D additionally max(#factor fields, #product groups) * nreplicas
+ * <= 65535 (pss_finalize returns PSS_EUNSUPPORTED otherwise).  The persistent 2D kernel runs the replicas two per launch. */
 int pss_set_replicas(pss_system *, int nreplicas);
 /* which replica pss_set_field / pss_get_field / pss_get_field_fourier / pss_debug_noise address (default 0) */
 int pss_select_replica(pss_system *, int replica);
@@ -92,7 +93,9 @@ int pss_replicas(const pss_system *);
 /* validate, freeze the term list, plan the kernels; *workspace_bytes = device bytes pss_bind needs. */
 int pss_finalize(pss_system *, size_t *workspace_bytes);
 /* device_workspace: DEVICE pointer, 256-byte aligned, >= workspace_bytes, zero-initialised by this
- * call.  cuda_stream: a cudaStream_t (NULL = default stream); all later work is issued on it. */
+ * call.  cuda_stream: a cudaStream_t of the workspace's device (NULL = default stream); all later work is issued on
+ * it.  The device that owns the workspace is recorded here; every later entry point makes it current for the
+ * duration of the call and restores the caller's current device, so the caller need not cudaSetDevice. */
 int pss_bind(pss_system *, void *device_workspace, size_t bytes, void *cuda_stream);
 /* R2C of user real data (x fastest) into the state.  on_device: 1 = DEVICE pointer, 0 = HOST pointer
  * (copied with cudaMemcpyAsync on the bound stream, then the stream is synchronised). */
@@ -109,6 +112,7 @@ int pss_get_field_fourier(pss_system *, int field, void *halfspectrum_out, int o
  * system and seed continues the run bit for bit (the noise is counter-based: SURVEY.md section 5).
  * halfspectrum_in: logical layout of pss_get_field_fourier, complex of the system precision. */
 int pss_set_field_fourier(pss_system *, int field, const void *halfspectrum_in, int on_device);
+/* PSS_ESTATE before pss_finalize. */
 int pss_set_step_count(pss_system *, uint64_t step);
 /* test hook for the noise stream (HOST pointers, either may be NULL): the 4 Philox4x32-10 words per
  * logical mode m, and the unit Hermitian Gaussian z (complex of the system precision) the step uses. */

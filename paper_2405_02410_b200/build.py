@@ -36,19 +36,5 @@ def build(force: bool = False, verbose: bool = False) -> str:
     return LIB
 
 
-COMPARE_SRC = os.path.join(HERE, "compare", "cufft_modelb.cu")
-COMPARE_LIB = os.path.join(HERE, "compare", "libpss_cufft_compare.so")
-
-
-def build_compare(force: bool = False) -> str:
-    """The cuFFT+cuRAND Model-B step (timing comparison for bench.py only; never loaded by the product)."""
-    if force or not os.path.exists(COMPARE_LIB) or os.path.getmtime(COMPARE_SRC) > os.path.getmtime(COMPARE_LIB):
-        nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-        tmp = COMPARE_LIB + ".tmp.%d" % os.getpid()
-        subprocess.run([nvcc] + NVCC_FLAGS + ["-o", tmp, COMPARE_SRC, "-lcufft", "-lcurand"], check=True)
-        os.replace(tmp, COMPARE_LIB)
-    return COMPARE_LIB
-
-
 if __name__ == "__main__":
     print(build(force=True, verbose=True))

@@ -69,6 +69,7 @@ struct pss_system {
   size_t off_state, off_psix, off_phat, off_scratch, off_ureal, off_tw[3], off_bar, ws_need;
   unsigned long long bar_count; /* value of the fused kernel's grid-barrier counter */
   char *ws;
+  int dev; /* device that owns the workspace (pss_bind); made current inside every entry point that launches */
   cudaStream_t stream;
   std::string cuda_msg;
   bool cuda_bad;
@@ -111,6 +112,16 @@ int cuda_fail(pss_system *s, cudaError_t e, const char *what) {
     if (e_ != cudaSuccess) return cuda_fail(s, e_, name);          \
     s->launches += 1;                                              \
   } while (0)
+
+/* makes the workspace's device current for the duration of an entry point and restores the caller's device */
+struct DeviceGuard {
+  int prev;
+  bool switched;
+  explicit DeviceGuard(int dev) : prev(-1), switched(false) {
+    if (dev >= 0 && cudaGetDevice(&prev) == cudaSuccess && prev != dev) switched = (cudaSetDevice(dev) == cudaSuccess);
+  }
+  ~DeviceGuard() { if (switched) cudaSetDevice(prev); }
+};
 
 int env_int(const char *name, int dflt) {
   const char *v = std::getenv(name);
@@ -460,6 +471,7 @@ int make_plan(pss_system *s) {
     }
     W = env_int("PSS_UPD_W", W);
     if (W < 1) W = 1;
+    if (W > 32) W = 32; /* the kernel keeps one keep-bit per line in a 32-bit mask */
     while (W & (W - 1)) W &= W - 1; /* a power of two (the kernel indexes with shifts) */
     while (W > 1 && per * W > SMEM_MAX) W >>= 1;
     pl.upd_W = W;
@@ -471,6 +483,9 @@ int make_plan(pss_system *s) {
     /* small lattices are latency-bound: at least n/2 threads (128..256) for the pointwise stage (measured) */
     if (n <= 512 && pl.upd_threads < 128) pl.upd_threads = (n >= 512) ? 256 : 128;
     pl.upd_threads = env_int("PSS_UPD_T", pl.upd_threads);
+    if (pl.upd_threads < 32) pl.upd_threads = 32;
+    if (pl.upd_threads > 256) pl.upd_threads = 256; /* __launch_bounds__(256) */
+    pl.upd_threads &= ~31;
   }
   /* k_rows: Wc pairs of rows per CTA (2*Wc contiguous rows of every kx) */
   if (P.ngrp > 0) {
@@ -501,15 +516,22 @@ int make_plan(pss_system *s) {
     if (pl.row_smem > 113 * 1024 && cs == 8 && (nx / 16) * Wc * (P.nfac > 0 ? P.nfac : 1) >= 512) pl.row_threads = 512;
     pl.row_threads = env_int("PSS_ROW_T", pl.row_threads);
     if (pl.row_threads > 512) pl.row_threads = 512;
+    if (pl.row_threads < 32) pl.row_threads = 32;
+    pl.row_threads &= ~31;
   }
   if (s->ndim == 3) {
     int W = env_int("PSS_MID_W", (int)(128 / cs));
+    if (W < 1) W = 1;
+    while (W & (W - 1)) W &= W - 1; /* a power of two, so that it divides nz */
     if (W > s->n[2]) W = (int)s->n[2];
     while ((size_t)W * pl.geo[1].npad * cs > SMEM_MAX && W > 1) W >>= 1;
     if ((size_t)W * pl.geo[1].npad * cs > SMEM_MAX) return PSS_EUNSUPPORTED;
     pl.mid_W = W;
     pl.mid_smem = (size_t)W * pl.geo[1].npad * cs;
     pl.mid_threads = env_int("PSS_MID_T", round_threads((s->n[1] / 32) * W)); /* two radix-16 butterflies per thread (measured) */
+    if (pl.mid_threads < 32) pl.mid_threads = 32;
+    if (pl.mid_threads > 256) pl.mid_threads = 256; /* __launch_bounds__(256) */
+    pl.mid_threads &= ~31;
   }
   return PSS_OK;
 }
@@ -898,17 +920,19 @@ template <typename T> int do_set_fourier(pss_system *s, int slot, const void *sr
 
 template <typename T> int do_debug_noise(pss_system *s, int field, uint64_t step, uint32_t *bits, void *z) {
   typedef typename cplx_of<T>::type C;
-  uint32_t *dbits = nullptr;
-  C *dz = nullptr;
-  if (bits) CK(cudaMalloc(&dbits, (size_t)s->M * 4 * sizeof(uint32_t)));
-  if (z) CK(cudaMalloc(&dz, (size_t)s->M * sizeof(C)));
-  k_debug_noise<T><<<592, 256, 0, s->stream>>>(s->P, (unsigned)s->sel, field, step, dbits, dz);
+  /* test hook: two temporary device buffers, released on every exit path */
+  struct Bufs {
+    uint32_t *dbits = nullptr;
+    C *dz = nullptr;
+    ~Bufs() { if (dbits) cudaFree(dbits); if (dz) cudaFree(dz); }
+  } b;
+  if (bits) CK(cudaMalloc(&b.dbits, (size_t)s->M * 4 * sizeof(uint32_t)));
+  if (z) CK(cudaMalloc(&b.dz, (size_t)s->M * sizeof(C)));
+  k_debug_noise<T><<<592, 256, 0, s->stream>>>(s->P, (unsigned)s->sel, field, step, b.dbits, b.dz);
   CKL("k_debug_noise");
-  if (bits) CK(cudaMemcpyAsync(bits, dbits, (size_t)s->M * 4 * sizeof(uint32_t), cudaMemcpyDeviceToHost, s->stream));
-  if (z) CK(cudaMemcpyAsync(z, dz, (size_t)s->M * sizeof(C), cudaMemcpyDeviceToHost, s->stream));
+  if (bits) CK(cudaMemcpyAsync(bits, b.dbits, (size_t)s->M * 4 * sizeof(uint32_t), cudaMemcpyDeviceToHost, s->stream));
+  if (z) CK(cudaMemcpyAsync(z, b.dz, (size_t)s->M * sizeof(C), cudaMemcpyDeviceToHost, s->stream));
   CK(cudaStreamSynchronize(s->stream));
-  if (dbits) cudaFree(dbits);
-  if (dz) cudaFree(dz);
   return PSS_OK;
 }
 
@@ -945,6 +969,7 @@ int pss_create(pss_system **out, int ndim, const int64_t n[3], const double dx[3
   s->N = s->n[0] * s->n[1] * s->n[2];
   s->M = (s->n[0] / 2 + 1) * s->n[1] * s->n[2];
   s->ws = nullptr;
+  s->dev = -1;
   s->stream = nullptr;
   s->cuda_bad = false;
   s->launches = 0;
@@ -1051,6 +1076,8 @@ int pss_finalize(pss_system *s, size_t *workspace_bytes) {
   if (rc != PSS_OK) return rc;
   rc = make_plan(s);
   if (rc != PSS_OK) return rc;
+  /* 3D: k_mid folds (array, replica) into gridDim.z (<= 65535) */
+  if (s->ndim == 3 && (long long)(s->P.nfac > s->P.ngrp ? s->P.nfac : s->P.ngrp) * s->nrep > 65535) return PSS_EUNSUPPORTED;
   carve_workspace(s);
   s->finalized = true;
   if (workspace_bytes) *workspace_bytes = s->ws_need;
@@ -1064,6 +1091,13 @@ int pss_bind(pss_system *s, void *device_workspace, size_t bytes, void *cuda_str
   int ndev = 0;
   CK(cudaGetDeviceCount(&ndev));
   if (ndev < 1) return cuda_fail(s, cudaErrorNoDevice, "pss_bind");
+  {
+    cudaPointerAttributes pa;
+    CK(cudaPointerGetAttributes(&pa, device_workspace));
+    if (pa.type != cudaMemoryTypeDevice && pa.type != cudaMemoryTypeManaged) return PSS_EINVAL;
+    s->dev = pa.device;
+  }
+  DeviceGuard guard(s->dev);
   s->ws = (char *)device_workspace;
   s->stream = (cudaStream_t)cuda_stream;
   CK(cudaMemsetAsync(s->ws, 0, s->ws_need, s->stream));
@@ -1082,6 +1116,7 @@ int pss_set_field(pss_system *s, int field, const void *real_xfastest, int on_de
   if (!s || !real_xfastest) return PSS_EINVAL;
   if (!s->finalized || !s->bound) return PSS_ESTATE;
   if (s->cuda_bad) return PSS_ECUDA;
+  DeviceGuard guard(s->dev);
   if (!fid_ok(s, field) || !s->fields[field].dynamic) return PSS_EINVAL;
   const int slot = s->dyn_slot[field];
   return (s->prec == PSS_F32) ? do_set_field<float>(s, slot, real_xfastest, on_device)
@@ -1092,6 +1127,7 @@ int pss_step(pss_system *s, int64_t nsteps) {
   if (!s || nsteps < 0) return PSS_EINVAL;
   if (!s->finalized || !s->bound) return PSS_ESTATE;
   if (s->cuda_bad) return PSS_ECUDA;
+  DeviceGuard guard(s->dev);
   return (s->prec == PSS_F32) ? do_steps<float>(s, nsteps) : do_steps<double>(s, nsteps);
 }
 
@@ -1099,6 +1135,7 @@ int pss_get_field(pss_system *s, int field, void *real_out, int on_device) {
   if (!s || !real_out) return PSS_EINVAL;
   if (!s->finalized || !s->bound) return PSS_ESTATE;
   if (s->cuda_bad) return PSS_ECUDA;
+  DeviceGuard guard(s->dev);
   if (!fid_ok(s, field) || !s->fields[field].dynamic) return PSS_EINVAL;
   const int slot = s->dyn_slot[field];
   return (s->prec == PSS_F32) ? do_get_field<float>(s, slot, real_out, on_device)
@@ -1109,6 +1146,7 @@ int pss_get_field_fourier(pss_system *s, int field, void *out, int on_device) {
   if (!s || !out) return PSS_EINVAL;
   if (!s->finalized || !s->bound) return PSS_ESTATE;
   if (s->cuda_bad) return PSS_ECUDA;
+  DeviceGuard guard(s->dev);
   if (!fid_ok(s, field) || !s->fields[field].dynamic) return PSS_EINVAL;
   const int slot = s->dyn_slot[field];
   return (s->prec == PSS_F32) ? do_get_fourier<float>(s, slot, out, on_device)
@@ -1119,6 +1157,7 @@ int pss_set_field_fourier(pss_system *s, int field, const void *in, int on_devic
   if (!s || !in) return PSS_EINVAL;
   if (!s->finalized || !s->bound) return PSS_ESTATE;
   if (s->cuda_bad) return PSS_ECUDA;
+  DeviceGuard guard(s->dev);
   if (!fid_ok(s, field) || !s->fields[field].dynamic) return PSS_EINVAL;
   const int slot = s->dyn_slot[field];
   return (s->prec == PSS_F32) ? do_set_fourier<float>(s, slot, in, on_device) : do_set_fourier<double>(s, slot, in, on_device);
@@ -1126,6 +1165,7 @@ int pss_set_field_fourier(pss_system *s, int field, const void *in, int on_devic
 
 int pss_set_step_count(pss_system *s, uint64_t step) {
   if (!s) return PSS_EINVAL;
+  if (!s->finalized) return PSS_ESTATE; /* the counter belongs to a finalized system (checkpoint/resume) */
   s->step = step;
   return PSS_OK;
 }
@@ -1134,6 +1174,7 @@ int pss_debug_noise(pss_system *s, int field, uint64_t step, uint32_t *bits, voi
   if (!s) return PSS_EINVAL;
   if (!s->finalized || !s->bound) return PSS_ESTATE;
   if (s->cuda_bad) return PSS_ECUDA;
+  DeviceGuard guard(s->dev);
   if (!fid_ok(s, field)) return PSS_EINVAL;
   return (s->prec == PSS_F32) ? do_debug_noise<float>(s, field, step, bits, z)
                               : do_debug_noise<double>(s, field, step, bits, z);
@@ -1143,6 +1184,7 @@ int pss_profile_step(pss_system *s, int64_t nsteps, double ms_per_launch[4], int
   if (!s || nsteps < 0 || nsteps > 4096 || !ms_per_launch || !launches) return PSS_EINVAL;
   if (!s->finalized || !s->bound) return PSS_ESTATE;
   if (s->cuda_bad) return PSS_ECUDA;
+  DeviceGuard guard(s->dev);
   if (s->ndim == 1) return PSS_EUNSUPPORTED;
   int rc = (s->prec == PSS_F32) ? do_steps<float>(s, 0) : do_steps<double>(s, 0);
   /* make sure the prologue (if any) is not inside the profiled region */

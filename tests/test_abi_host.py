@@ -39,8 +39,8 @@ def test_product_does_not_reference_the_oracle():
 
 
 def test_comparison_build_exports_its_symbol(pss):
-    from paper_2405_02410_b200 import build
-    lib = ctypes.CDLL(build.build_compare())
+    from compare import build as compare_build
+    lib = ctypes.CDLL(compare_build.build())
     assert hasattr(lib, "cmp_cufft_modelb")
 
 

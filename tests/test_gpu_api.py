@@ -161,3 +161,35 @@ def test_checkpoint_resume_is_bit_identical(pss, name, n):
         ref = b.get_field_fourier(f).view(np.uint32)
         assert np.array_equal(a.get_field_fourier(f).view(np.uint32), ref)
         assert np.array_equal(c.get_field_fourier(f).view(np.uint32), ref)
+
+
+def test_system_on_a_device_that_is_not_current(pss):
+    """the library records the workspace's device in pss_bind and makes it current inside every entry
+    point.  With two or more GPUs: build on cuda:1 while cuda:0 is current; with one GPU: the guard is a no-op and the
+    call sequence is checked with an explicit (non-default) stream."""
+    import torch
+    from paper_2405_02410_b200 import workloads as wl
+    cfg = wl.make_config("modelb_128", n=(64, 64))
+    ref, ids = wl.build(pss, cfg, prec="f32")
+    ref.step(5)
+    want = ref.get_field_fourier(ids["phi"])
+    if torch.cuda.device_count() >= 2:
+        torch.cuda.set_device(0)
+        g, _ = wl.build(pss, cfg, prec="f32", device="cuda:1")
+        g.step(5)
+        assert torch.cuda.current_device() == 0
+    else:
+        st = torch.cuda.Stream()
+        g, _ = wl.build(pss, cfg, prec="f32", stream=st)
+        g.step(5)
+    got = g.get_field_fourier(ids["phi"])
+    assert np.array_equal(got.view(np.uint32), want.view(np.uint32))
+
+
+def test_set_step_count_needs_a_finalized_system(pss):
+    b = pss.binding
+    s = pss.System((64, 64), (1.0, 1.0), 0.01)
+    s.add_field("phi", True)
+    with pytest.raises(b.PssError) as e:
+        s.set_step_count(3)
+    assert e.value.code == b.ESTATE

@@ -12,8 +12,10 @@ from paper_2405_02410_b200 import workloads as wl
 
 pytestmark = pytest.mark.gpu
 
-TOL1 = {"f32": 1e-5, "f64": 1e-12}
-TOLN = {"f32": 1e-3, "f64": 1e-9}
+import os
+
+import parity_util as pu
+from parity_util import TOL1, TOLN, rel_l2
 
 
 @pytest.fixture(scope="module")
@@ -25,43 +27,23 @@ def pss():
     return p
 
 
-def rel_l2(a, b):
-    a = np.asarray(a, dtype=np.float64)
-    b = np.asarray(b, dtype=np.float64)
-    den = np.linalg.norm(b.ravel())
-    return np.linalg.norm((a - b).ravel()) / (den if den > 0 else 1.0)
-
-
 def both(pss, oracle, cfg, prec):
-    g, ids = wl.build(pss, cfg, prec=prec)
-    o, ids_o = wl.build(oracle, cfg, prec=prec)
-    assert ids == ids_o
-    return g, o, [ids[name] for name in cfg["ic"].keys()]
+    return pu.both(wl, pss, oracle, cfg, prec)
 
 
 def check(g, o, dyn, tol, what):
-    worst = 0.0
-    for f in dyn:
-        a, b = g.get_field(f), o.get_field(f)
-        assert np.all(np.isfinite(a)), what
-        e = rel_l2(a, b)
-        worst = max(worst, e)
-        assert e <= tol, "%s: field %d rel L2 %.3e > %.1e" % (what, f, e, tol)
-    print("%s: rel L2 %.3e (tol %.1e)" % (what, worst, tol))
-    return worst
+    return pu.compare_fields(g, o, dyn, tol, what)
 
 
 def run_horizons(pss, oracle, cfg, prec, horizons, what):
-    """horizons: [(total steps, tolerance), ...] increasing; each increment is ONE pss_step(n) call."""
-    g, o, dyn = both(pss, oracle, cfg, prec)
-    done = 0
-    for total, tol in horizons:
-        g.step(total - done)
-        o.step(total - done)
-        done = total
-        assert g.step_count == total
-        check(g, o, dyn, tol, "%s %s, %d steps" % (what, prec, total))
-    return g
+    return pu.run_horizons(wl, pss, oracle, cfg, prec, horizons, what)
+
+
+# Long horizon of the two configurations whose oracle takes minutes per 1000 steps (256^3: ~2.4 steps/s, KPZ 4096^2:
+# ~1.3 steps/s on 16 cores).  Default: 200 / 100 steps at FULL size so that the whole `-m gpu` suite stays inside the
+# driver's time limit; the 1000-step tolerance itself is tested on 64^3 / 512^2 in test_gpu_parity.py, and
+# PSS_FULL_HORIZON=1000 runs the full-size comparison to 1000 steps (result recorded in DESIGN.md section 3).
+FULL_HORIZON = int(os.environ.get("PSS_FULL_HORIZON", "0"))
 
 
 # config 2: 2D Model B 1024^2, fp32 (the headline; persistent fused kernel) and fp64 (generic kernels)
@@ -99,7 +81,8 @@ def test_config2_other_dealias_rules_full_size(pss, oracle):
 # config 3: 3D Model B 256^3 fp32
 def test_config3_modelb_256_cubed(pss, oracle):
     cfg = wl.make_config("modelb_256c")
-    run_horizons(pss, oracle, cfg, "f32", [(1, TOL1["f32"]), (10, 10 * TOL1["f32"])], "config 3 (256^3)")
+    n = FULL_HORIZON or 200
+    run_horizons(pss, oracle, cfg, "f32", [(1, TOL1["f32"]), (10, 10 * TOL1["f32"]), (n, TOLN["f32"])], "config 3 (256^3)")
 
 
 # config 4: nematic 1024^2 fp32, parity horizon 250 steps (A20)
@@ -111,7 +94,8 @@ def test_config4_nematic_1024(pss, oracle):
 # config 5: KPZ 4096^2 fp32
 def test_config5_kpz_4096(pss, oracle):
     cfg = wl.make_config("kpz_4096")
-    run_horizons(pss, oracle, cfg, "f32", [(1, TOL1["f32"]), (20, 10 * TOL1["f32"])], "config 5 (KPZ 4096^2)")
+    n = FULL_HORIZON or 100
+    run_horizons(pss, oracle, cfg, "f32", [(1, TOL1["f32"]), (20, 10 * TOL1["f32"]), (n, TOLN["f32"])], "config 5 (KPZ 4096^2)")
 
 
 # config 5b: the Model-B lattice sweep 256^2 .. 8192^2

@@ -11,8 +11,8 @@ from paper_2405_02410_b200 import workloads as wl
 
 pytestmark = pytest.mark.gpu
 
-TOL1 = {"f32": 1e-5, "f64": 1e-12}
-TOLN = {"f32": 1e-3, "f64": 1e-9}
+import parity_util as pu
+from parity_util import TOL1, TOLN, rel_l2, compare_fields
 
 
 @pytest.fixture(scope="module")
@@ -24,30 +24,8 @@ def pss():
     return p
 
 
-def rel_l2(a, b):
-    a = np.asarray(a, dtype=np.float64)
-    b = np.asarray(b, dtype=np.float64)
-    den = np.linalg.norm(b.ravel())
-    return np.linalg.norm((a - b).ravel()) / (den if den > 0 else 1.0)
-
-
 def both(pss, oracle, cfg, prec, dealias=None):
-    g, ids = wl.build(pss, cfg, prec=prec, dealias=dealias)
-    o, ids_o = wl.build(oracle, cfg, prec=prec, dealias=dealias)
-    assert ids == ids_o
-    dyn = [ids[name] for name in cfg["ic"].keys()]
-    return g, o, dyn
-
-
-def compare_fields(g, o, dyn, tol, what):
-    worst = 0.0
-    for f in dyn:
-        a, b = g.get_field(f), o.get_field(f)
-        assert np.all(np.isfinite(a)), what
-        e = rel_l2(a, b)
-        worst = max(worst, e)
-        assert e <= tol, "%s: field %d rel L2 %.3e > %.1e" % (what, f, e, tol)
-    return worst
+    return pu.both(wl, pss, oracle, cfg, prec, dealias)
 
 
 # ---------------------------------------------------------------------------------------------
@@ -157,6 +135,17 @@ def test_config1_modelb_128_1000_steps(pss, oracle, prec):
     print("config1 %s 1000 steps rel L2 %.3e" % (prec, e))
 
 
+# ---------------------------------------------------------------------------------------------
+# the 1000-step tolerance on the 3D path (k_mid) and the KPZ path (odd-derivative factors), reduced lattices:
+# PAPER.md:128-135 iterated 1000 times, north_star's <= 1e-3 (fp32) / <= 1e-9 (fp64)
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("name,n", [("modelb_256c", (64, 64, 64)), ("kpz_4096", (512, 512))])
+@pytest.mark.parametrize("prec", ["f32", "f64"])
+def test_1000_steps_3d_and_kpz_reduced(pss, oracle, name, n, prec):
+    cfg = wl.make_config(name, n=n)
+    pu.run_horizons(wl, pss, oracle, cfg, prec, [(1, TOL1[prec]), (1000, TOLN[prec])], "%s %s" % (name, n))
+
+
 def test_nematic_horizon_250_steps(pss, oracle):
     """A20: config 4 is chaotic; the parity horizon is 250 steps (here on 128^2)."""
     cfg = wl.make_config("nematic_1024", n=(128, 128))
@@ -211,8 +200,8 @@ def test_p8_philox_matches_curand_device_api(pss, oracle):
     """P8: the oracle's Philox4x32-10 block and the words the CUDA path draws equal cuRAND's device
     generator (curand_init + curand4) for the same key and counter — an implementation neither side wrote."""
     import ctypes
-    from paper_2405_02410_b200 import build
-    lib = ctypes.CDLL(build.build_compare())
+    from compare import build as compare_build
+    lib = ctypes.CDLL(compare_build.build())
     lib.cmp_curand_philox_block.argtypes = [ctypes.c_uint64, ctypes.c_uint64, ctypes.c_uint64, ctypes.POINTER(ctypes.c_uint32)]
 
     def curand_block(ctr, key):

@@ -330,6 +330,49 @@ def test_p7_noise_amplitude_real_space_variance(oracle):
     assert v == pytest.approx(2 * D * dt / (dx[0] * dx[1]), rel=0.12)
 
 
+@pytest.mark.parametrize("a", [-2, -1, 1, 2, 3])
+@pytest.mark.parametrize("n,dx", [((16, 8), (0.5, 1.25)), ((8, 4, 4), (1.0, 0.7, 2.0)), ((32,), (0.3,))])
+def test_p7_noise_amplitude_odd_and_negative_q_powers(oracle, a, n, dx):
+    """noise prefactor "a power of q^2 and 1/q" (reading A13: D~ = D |q|^a, any integer a), with
+    L = 0 and no rhs: one step from 0 gives phi_q = nu_q (Eq. 18), so
+      (i)  mode by mode  phi_q / z_q = sqrt(2 D |q|^a dt N / dV)  (z_q: the unit Hermitian Gaussian pinned by P7;
+           PAPER.md:113 Eq. 16 with reading A1), 0 at q = 0 for a < 0 (A10), and
+      (ii) averaged over seeds  <|phi_q|^2> = 2 D |q|^a dt N / dV.
+    |q| is written out here from the integer mode numbers (q_j = 2 pi s(k_j) / (N_j dx_j), Nyquist index -> pi/dx_j)."""
+    dt, D = 0.02, 0.7
+    ndim = len(n)
+    N, dV = float(np.prod(n)), float(np.prod(dx))
+    qs = []
+    for j in range(ndim):
+        k = np.arange(n[j] // 2 + 1) if j == 0 else np.fft.fftfreq(n[j], 1.0 / n[j])
+        qs.append(2 * np.pi * np.abs(k) / (n[j] * dx[j]))
+    grids = np.meshgrid(*qs[::-1], indexing="ij")            # slowest axis first, x last (the half-spectrum layout)
+    qabs = np.sqrt(sum(g * g for g in grids))
+    with np.errstate(divide="ignore"):
+        qa = np.where(qabs > 0, qabs ** float(a), 0.0 if a < 0 else (1.0 if a == 0 else 0.0))
+    amp2 = 2 * D * qa * dt * N / dV
+    acc = np.zeros_like(amp2)
+    nseed = 160
+    for seed in range(nseed):
+        s = oracle.System(n, dx, dt, prec="f64", seed=1000 + seed)
+        f = s.add_field("phi", True)
+        s.set_noise(f, D, a)
+        s.finalize()
+        s.set_field(f, np.zeros(n[::-1]))
+        s.step(1)
+        spec = s.get_field_fourier_f64(f)
+        if seed < 3:
+            _, z = s.debug_noise(f, 0)
+            assert np.abs(spec - np.sqrt(amp2) * z).max() <= 1e-12 * max(1.0, np.sqrt(amp2).max())
+            if a < 0:
+                assert spec.flat[0] == 0.0
+        acc += np.abs(spec) ** 2
+    sel = amp2 > 0
+    ratio = (acc / nseed)[sel] / amp2[sel]
+    assert abs(ratio.mean() - 1.0) < 5.0 / math.sqrt(nseed * sel.sum())
+    assert np.abs(ratio - 1.0).max() < 0.6                  # 160 samples per mode (chi^2 with 1-2 dof)
+
+
 # ------------------------------------------------------------------------------------------ P9
 def test_p9_odd_derivative_nyquist_and_inverse_q(oracle):
     nx, ny, dx = 16, 8, 0.5
