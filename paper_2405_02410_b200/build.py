@@ -12,7 +12,7 @@ INCLUDE = os.path.join(os.path.dirname(HERE), "include")
 LIB = os.path.join(HERE, "libpss.so")
 SOURCES = [os.path.join(CSRC, "pss.cu")]
 DEPS = SOURCES + [os.path.join(CSRC, f) for f in
-                  ("pss_program.h", "pss_fft.cuh", "pss_pointwise.cuh", "pss_kernels.cuh", "pss_fused2d.cuh")] + \
+                  ("pss_program.h", "pss_fft.cuh", "pss_pointwise.cuh", "pss_kernels.cuh", "pss_fused2d.cuh", "pss_persist2d.cuh")] + \
     [os.path.join(INCLUDE, "pss.h")]
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",

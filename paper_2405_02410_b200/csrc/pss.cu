@@ -8,6 +8,7 @@
  */
 #include "../../include/pss.h"
 
+#include <algorithm>
 #include <cmath>
 #include <cstdio>
 #include <cstdlib>
@@ -17,6 +18,7 @@
 
 #include "pss_kernels.cuh"
 #include "pss_fused2d.cuh"
+#include "pss_persist2d.cuh"
 
 namespace {
 
@@ -43,6 +45,7 @@ struct Plan {
   int fused_prune;                  /* its input-pruned instantiation (mask cutoff <= n/4 on both axes)       */
   int pdl;                          /* programmatic dependent launch between the step kernels (PSS_PDL=0 disables) */
   int fused_pair;                   /* ensembles: two replicas per launch (k_fused2d_pair)                    */
+  int persist;                      /* 1: pss_persist2d.cuh's kernel (cutoff <= N/4: bulk-copy exchanges) runs single systems (PSS_PERSIST=0 disables) */
 };
 
 }  // namespace
@@ -549,7 +552,7 @@ void carve_workspace(pss_system *s) {
   s->off_scratch = off; off += arr;
   s->off_ureal = off; off += align_up((size_t)s->N * s->rsize, 256);
   for (int j = 0; j < 3; ++j) { s->off_tw[j] = off; off += align_up((size_t)tw_entries(s->plan.geo[j]) * s->csize, 256); }
-  s->off_bar = off; off += 256;
+  s->off_bar = off; off += 512; /* first-generation counter | the two counters of pss_persist2d.cuh */
   s->ws_need = off;
 }
 
@@ -595,6 +598,13 @@ int setup_fused(pss_system *s) {
   else
     CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, f2d::k_fused2d<false>, f2d::THREADS, f2d::SMEM_BYTES));
   if (!coop || (long long)occ * nsm < f2d::NCTA) s->plan.fused = 0;
+  s->plan.persist = 0;
+  if (s->plan.fused && s->plan.fused_prune && env_int("PSS_PERSIST", 1) != 0) {
+    int occ3 = 0;
+    CK(cudaFuncSetAttribute(p2d::k_persist2d, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p2d::SMEM_BYTES));
+    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ3, p2d::k_persist2d, p2d::THREADS, p2d::SMEM_BYTES));
+    if ((long long)occ3 * nsm >= p2d::NCTA) s->plan.persist = 1;
+  }
   /* ensembles: the two-replica kernel needs more shared memory; fall back to one launch per replica if it does not fit */
   s->plan.fused_pair = 0;
   if (s->plan.fused && s->nrep >= 2 && env_int("PSS_FUSED_PAIR", 1) != 0) {
@@ -768,13 +778,46 @@ int launch_fused(pss_system *s, int64_t nsteps) {
     a.prologue = prologue;
     a.rep_stride = arr_stride(s); /* ndyn = nfac = ngrp = 1: consecutive replicas are one array apart */
     void *params[2] = {(void *)&Pr, (void *)&a};
-    prof_mark(s, KIND_FUSED, true);
-    cudaError_t e = cudaLaunchCooperativeKernel(pair ? fn2 : fn1, dim3(f2d::NCTA), dim3(f2d::THREADS), params,
-                                                pair ? f2d::SMEM_BYTES_PAIR : f2d::SMEM_BYTES, s->stream);
-    prof_mark(s, KIND_FUSED, false);
-    if (e != cudaSuccess) return cuda_fail(s, e, "k_fused2d");
-    CKL("k_fused2d");
-    s->bar_count += (unsigned long long)f2d::NCTA * (unsigned long long)(2 * nsteps + prologue);
+    cudaError_t e;
+    if (!pair && s->plan.persist) {
+      /* second-generation kernel: its two barrier counters start from zero in every launch */
+      p2d::Args pa;
+      pa.state = a.state; pa.Eg = a.E; pa.Zg = a.Z; pa.tw = a.tw;
+      pa.bar = a.bar + 32; /* 256 bytes past the first-generation counter */
+      pa.nsteps = nsteps; pa.step0 = s->step; pa.prologue = prologue;
+      pa.dbg = env_int("PSS_P2D_DBG", 0);
+      pa.ts = env_int("PSS_P2D_TS", 0) ? reinterpret_cast<long long *>(s->ws + s->off_scratch) : nullptr;
+      CK(cudaMemsetAsync(pa.bar, 0, 256, s->stream));
+      void *pparams[2] = {(void *)&Pr, (void *)&pa};
+      prof_mark(s, KIND_FUSED, true);
+      e = cudaLaunchCooperativeKernel((const void *)p2d::k_persist2d, dim3(p2d::NCTA), dim3(p2d::THREADS), pparams, p2d::SMEM_BYTES, s->stream);
+      prof_mark(s, KIND_FUSED, false);
+      if (e != cudaSuccess) return cuda_fail(s, e, "k_persist2d");
+      CKL("k_persist2d");
+      if (pa.ts && nsteps >= 3) { /* timing experiment: print the stamps of a few CTAs */
+        std::vector<long long> h(129 * 2 * 32);
+        cudaStreamSynchronize(s->stream);
+        cudaMemcpy(h.data(), pa.ts, h.size() * sizeof(long long), cudaMemcpyDeviceToHost);
+        /* globaltimer stamps: per stamp the min / median / max over all groups, relative to the earliest stamp 0 */
+        long long t00 = -1;
+        for (int c = 0; c < 128; ++c) for (int g = 0; g < 2; ++g) { const long long v = h[(c * 2 + g) * 32]; if (v && (t00 < 0 || v < t00)) t00 = v; }
+        for (int i = 0; i < 18; ++i) {
+          std::vector<long long> v;
+          for (int c = 0; c < 129; ++c) for (int g = 0; g < 2; ++g) if (h[(c * 2 + g) * 32 + i]) v.push_back(h[(c * 2 + g) * 32 + i] - t00);
+          if (v.empty()) continue;
+          std::sort(v.begin(), v.end());
+          std::printf("stamp %2d: n=%3d min %6lld med %6lld max %6lld ns\n", i, (int)v.size(), v.front(), v[v.size() / 2], v.back());
+        }
+      }
+    } else {
+      prof_mark(s, KIND_FUSED, true);
+      e = cudaLaunchCooperativeKernel(pair ? fn2 : fn1, dim3(f2d::NCTA), dim3(f2d::THREADS), params,
+                                      pair ? f2d::SMEM_BYTES_PAIR : f2d::SMEM_BYTES, s->stream);
+      prof_mark(s, KIND_FUSED, false);
+      if (e != cudaSuccess) return cuda_fail(s, e, "k_fused2d");
+      CKL("k_fused2d");
+      s->bar_count += (unsigned long long)f2d::NCTA * (unsigned long long)(2 * nsteps + prologue);
+    }
     r += pair ? 2 : 1;
   }
   s->psix_valid = true;
