@@ -552,7 +552,7 @@ void carve_workspace(pss_system *s) {
   s->off_scratch = off; off += arr;
   s->off_ureal = off; off += align_up((size_t)s->N * s->rsize, 256);
   for (int j = 0; j < 3; ++j) { s->off_tw[j] = off; off += align_up((size_t)tw_entries(s->plan.geo[j]) * s->csize, 256); }
-  s->off_bar = off; off += 512; /* first-generation counter | the two counters of pss_persist2d.cuh */
+  s->off_bar = off; off += 256;
   s->ws_need = off;
 }
 
@@ -599,12 +599,13 @@ int setup_fused(pss_system *s) {
     CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, f2d::k_fused2d<false>, f2d::THREADS, f2d::SMEM_BYTES));
   if (!coop || (long long)occ * nsm < f2d::NCTA) s->plan.fused = 0;
   s->plan.persist = 0;
-  if (s->plan.fused && s->plan.fused_prune && env_int("PSS_PERSIST", 1) != 0) {
+  if (s->plan.fused && s->plan.fused_prune && s->nrep == 1 && env_int("PSS_PERSIST", 1) != 0) {
     int occ3 = 0;
     CK(cudaFuncSetAttribute(p2d::k_persist2d, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p2d::SMEM_BYTES));
     CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ3, p2d::k_persist2d, p2d::THREADS, p2d::SMEM_BYTES));
     if ((long long)occ3 * nsm >= p2d::NCTA) s->plan.persist = 1;
   }
+
   /* ensembles: the two-replica kernel needs more shared memory; fall back to one launch per replica if it does not fit */
   s->plan.fused_pair = 0;
   if (s->plan.fused && s->nrep >= 2 && env_int("PSS_FUSED_PAIR", 1) != 0) {
@@ -780,25 +781,38 @@ int launch_fused(pss_system *s, int64_t nsteps) {
     void *params[2] = {(void *)&Pr, (void *)&a};
     cudaError_t e;
     if (!pair && s->plan.persist) {
-      /* second-generation kernel: its two barrier counters start from zero in every launch */
+      /* second-generation kernel (pss_persist2d.cuh): flag-in-data exchanges, no barrier counters */
       p2d::Args pa;
-      pa.state = a.state; pa.Eg = a.E; pa.Zg = a.Z; pa.tw = a.tw;
-      pa.bar = a.bar + 32; /* 256 bytes past the first-generation counter */
+      pa.state = a.state;
+      pa.Ex = a.E; /* the factor array and the group array serve as the two exchange buffers */
+      pa.Zx = a.Z;
+      pa.w512 = a.bar + 16;
+      pa.tw = a.tw;
       pa.nsteps = nsteps; pa.step0 = s->step; pa.prologue = prologue;
+      pa.ts = nullptr;
       pa.dbg = env_int("PSS_P2D_DBG", 0);
+#ifdef PSS_P2D_DEBUG
       pa.ts = env_int("PSS_P2D_TS", 0) ? reinterpret_cast<long long *>(s->ws + s->off_scratch) : nullptr;
-      CK(cudaMemsetAsync(pa.bar, 0, 256, s->stream));
+#endif
+      CK(cudaMemsetAsync(pa.w512, 0, 8, s->stream));
+      if (prologue) { /* stale buffers: every word gets the parity of step0 - 1, i.e. "not written yet" for step0 */
+        const uint32_t lsb = (uint32_t)((s->step & 1ull) ^ 1ull);
+        p2d::k_fill_tag<<<296, 256, 0, s->stream>>>(reinterpret_cast<uint32_t *>(pa.Zx), p2d::ZX_ELEMS * 2, lsb);
+        CKL("k_fill_tag");
+        p2d::k_fill_tag<<<296, 256, 0, s->stream>>>(reinterpret_cast<uint32_t *>(pa.Ex), p2d::EX_ELEMS * 2, lsb);
+        CKL("k_fill_tag");
+      }
       void *pparams[2] = {(void *)&Pr, (void *)&pa};
       prof_mark(s, KIND_FUSED, true);
       e = cudaLaunchCooperativeKernel((const void *)p2d::k_persist2d, dim3(p2d::NCTA), dim3(p2d::THREADS), pparams, p2d::SMEM_BYTES, s->stream);
       prof_mark(s, KIND_FUSED, false);
       if (e != cudaSuccess) return cuda_fail(s, e, "k_persist2d");
       CKL("k_persist2d");
-      if (pa.ts && nsteps >= 3) { /* timing experiment: print the stamps of a few CTAs */
+#ifdef PSS_P2D_DEBUG
+      if (pa.ts && nsteps >= 3) { /* timing experiment: globaltimer stamps, min / median / max over all groups */
         std::vector<long long> h(129 * 2 * 32);
         cudaStreamSynchronize(s->stream);
         cudaMemcpy(h.data(), pa.ts, h.size() * sizeof(long long), cudaMemcpyDeviceToHost);
-        /* globaltimer stamps: per stamp the min / median / max over all groups, relative to the earliest stamp 0 */
         long long t00 = -1;
         for (int c = 0; c < 128; ++c) for (int g = 0; g < 2; ++g) { const long long v = h[(c * 2 + g) * 32]; if (v && (t00 < 0 || v < t00)) t00 = v; }
         for (int i = 0; i < 18; ++i) {
@@ -809,6 +823,7 @@ int launch_fused(pss_system *s, int64_t nsteps) {
           std::printf("stamp %2d: n=%3d min %6lld med %6lld max %6lld ns\n", i, (int)v.size(), v.front(), v[v.size() / 2], v.back());
         }
       }
+#endif
     } else {
       prof_mark(s, KIND_FUSED, true);
       e = cudaLaunchCooperativeKernel(pair ? fn2 : fn1, dim3(f2d::NCTA), dim3(f2d::THREADS), params,
@@ -1209,6 +1224,7 @@ int pss_set_field_fourier(pss_system *s, int field, const void *in, int on_devic
 int pss_set_step_count(pss_system *s, uint64_t step) {
   if (!s) return PSS_EINVAL;
   if (!s->finalized) return PSS_ESTATE; /* the counter belongs to a finalized system (checkpoint/resume) */
+  if (step != s->step) s->psix_valid = false; /* the persistent kernel's exchange buffers are indexed by the step parity */
   s->step = step;
   return PSS_OK;
 }
