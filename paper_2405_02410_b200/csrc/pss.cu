@@ -552,7 +552,7 @@ void carve_workspace(pss_system *s) {
   s->off_scratch = off; off += arr;
   s->off_ureal = off; off += align_up((size_t)s->N * s->rsize, 256);
   for (int j = 0; j < 3; ++j) { s->off_tw[j] = off; off += align_up((size_t)tw_entries(s->plan.geo[j]) * s->csize, 256); }
-  s->off_bar = off; off += 256;
+  s->off_bar = off; off += 512; /* first-generation counter | the two counters of pss_persist2d.cuh */
   s->ws_need = off;
 }
 
@@ -784,24 +784,19 @@ int launch_fused(pss_system *s, int64_t nsteps) {
       /* second-generation kernel (pss_persist2d.cuh): flag-in-data exchanges, no barrier counters */
       p2d::Args pa;
       pa.state = a.state;
-      pa.Ex = a.E; /* the factor array and the group array serve as the two exchange buffers */
-      pa.Zx = a.Z;
-      pa.w512 = a.bar + 16;
+      pa.Eg = a.E; /* the factor array and the group array hold the two exchange arrays */
+      pa.Zg = a.Z;
       pa.tw = a.tw;
+      pa.bar = a.bar + 32; /* 256 bytes past the first-generation counter; its two counters start from zero in every launch */
       pa.nsteps = nsteps; pa.step0 = s->step; pa.prologue = prologue;
-      pa.ts = nullptr;
+      pa.gate = env_int("PSS_NOISE_GATE", 1);
+      pa.prio = env_int("PSS_P2D_PRIO", 1);
       pa.dbg = env_int("PSS_P2D_DBG", 0);
+      pa.ts = nullptr;
 #ifdef PSS_P2D_DEBUG
       pa.ts = env_int("PSS_P2D_TS", 0) ? reinterpret_cast<long long *>(s->ws + s->off_scratch) : nullptr;
 #endif
-      CK(cudaMemsetAsync(pa.w512, 0, 8, s->stream));
-      if (prologue) { /* stale buffers: every word gets the parity of step0 - 1, i.e. "not written yet" for step0 */
-        const uint32_t lsb = (uint32_t)((s->step & 1ull) ^ 1ull);
-        p2d::k_fill_tag<<<296, 256, 0, s->stream>>>(reinterpret_cast<uint32_t *>(pa.Zx), p2d::ZX_ELEMS * 2, lsb);
-        CKL("k_fill_tag");
-        p2d::k_fill_tag<<<296, 256, 0, s->stream>>>(reinterpret_cast<uint32_t *>(pa.Ex), p2d::EX_ELEMS * 2, lsb);
-        CKL("k_fill_tag");
-      }
+      CK(cudaMemsetAsync(pa.bar, 0, 256, s->stream));
       void *pparams[2] = {(void *)&Pr, (void *)&pa};
       prof_mark(s, KIND_FUSED, true);
       e = cudaLaunchCooperativeKernel((const void *)p2d::k_persist2d, dim3(p2d::NCTA), dim3(p2d::THREADS), pparams, p2d::SMEM_BYTES, s->stream);
@@ -1224,7 +1219,6 @@ int pss_set_field_fourier(pss_system *s, int field, const void *in, int on_devic
 int pss_set_step_count(pss_system *s, uint64_t step) {
   if (!s) return PSS_EINVAL;
   if (!s->finalized) return PSS_ESTATE; /* the counter belongs to a finalized system (checkpoint/resume) */
-  if (step != s->step) s->psix_valid = false; /* the persistent kernel's exchange buffers are indexed by the step parity */
   s->step = step;
   return PSS_OK;
 }

@@ -4,21 +4,17 @@
  *
  * What changed against pss_fused2d.cuh (which stays for the other de-aliasing rules and for replica pairs).  The
  * timeline of that kernel (globaltimer stamps, profiles/r2_persist2d.md) showed half of the step in the two all-to-all
- * exchanges: per exchange ~0.5 us of stores, ~0.6 us in the release fence of the grid barrier, ~0.6 us until the last
- * arrival is seen by the pollers, ~0.7 us for the dependent loads.  Here
+ * exchanges, and its per-thread 8-byte global accesses touching 4-8 different 128-byte lines per warp instruction.
+ * Here
  *   - each exchange array is laid out per CONSUMER CTA as one contiguous block made of 128-byte chunks, one chunk per
  *     producer: the producer writes whole lines (16 bytes per lane), the consumer reads its block with fully
  *     coalesced 16-byte loads; the transposition happens in shared memory on both sides (scatter into a staging tile /
  *     gather out of it) with an in-chunk rotation that makes every half-warp access hit 16 different banks;
- *   - there is NO grid barrier and no fence: the data carry their own validity.  The least significant mantissa bit
- *     of every 32-bit word written to an exchange buffer is replaced by the parity of the step that consumes it
- *     (values are exchanged with a 23-bit mantissa: one extra rounding of 2^-23 relative per exchange, accounted for
- *     in DESIGN.md's tolerance budget).  A buffer is rewritten every step, so its previous content carries the other
- *     parity: the consumer polls its block with relaxed gpu-scope loads until every word shows the parity it waits
- *     for.  Observing a word IS receiving it (single-location coherence): no ordering between different locations,
- *     no atomicity of wider accesses, no reset traffic.  A producer can only overwrite a block after its consumer has
- *     read it, because the producer's own next input depends on that consumer's output (column 512, which feeds
- *     nothing back, publishes a progress word instead).  See DESIGN.md section 6;
+ *   - the consumer fetches its block with 16-byte asynchronous copies (cp.async.cg, global -> shared, no registers)
+ *     issued by all 256 transform threads as soon as the one polling thread has seen the grid barrier open;
+ *   - the noise warps draw z(s+1) while the transform warps WAIT (grid barrier in flight, block being fetched) and
+ *     pause while they compute: the step is issue-bound in its compute phases and latency-bound in its exchanges, so
+ *     the third of the instructions that is noise goes where the issue slots are free;
  *   - a CTA's 256 transform threads are two independent 128-thread groups (2 lines each) with their own named
  *     barriers, so one group's exchange traffic overlaps the other's transforms; group 0 owns the two de-aliased
  *     (kept) columns, whose inverse transform feeds the next exchange, group 1 the two columns outside the mask.
@@ -36,11 +32,11 @@
  *   phase R (rows, x axis):    group (b, g) owns the packed row pairs p = 4 b + 2 g + L        ("bg" = 2 b + g)
  *   phase C (columns, y axis): group (c, gc) owns the columns kx = 256 gc + 2 c + L;  CTA 128 owns kx = 512
  *
- * Exchange buffers (float2; two of each, indexed by the parity of the step that consumes them):
- *   Zx [c in 0..127][bg in 0..255][16]   chunk (bg -> c): Z[k'][p] for p = 2 bg + L and the eight k' CTA c consumes,
+ * Exchange arrays (float2):
+ *   Zg [c in 0..127][bg in 0..255][16]   chunk (bg -> c): Z[k'][p] for p = 2 bg + L and the eight k' CTA c consumes,
  *       element (gc, L, s) at (8 gc + 4 L + s + 2 c + rho(bg)) & 15, s = 0,1: kx = 256 gc + 2 c + s, s = 2,3: its
  *       mirror 1024 - kx;  rho(bg) = (bg & 3) | ((bg & 4) << 1).   Z512[p] for column 512 follows the 128 blocks.
- *   Ex [b in 0..127][c in 0..127][16]    chunk (c -> b): E[p][k'] for p = 4 b + pl and kx = 2 c + s (s = 0,1) and the
+ *   Eg [b in 0..127][c in 0..127][16]    chunk (c -> b): E[p][k'] for p = 4 b + pl and kx = 2 c + s (s = 0,1) and the
  *       mirrors (s = 2,3), element (pl, s) at (4 pl + s + 2 c + b) & 15.
  *   Producers: lanes walk consecutive k (2 c + s) -> 16 banks.  Consumers of Z: lanes walk (bg, L) -> 4 L + rho(bg);
  *   consumers of E: lanes walk consecutive k again.  Every staging index below is a thread constant plus a
@@ -62,19 +58,21 @@ constexpr int PITCH = 65;             /* k1-row pitch of an exchange buffer (flo
 constexpr int BUF = 16 * PITCH;       /* one line's exchange buffer                        */
 constexpr int REGA = 4096;            /* staging A (float2): Z out (two groups x 2048) in phase R, Z in (4096) in phase C */
 constexpr int REGB = 2048;            /* staging B (float2): E in (phase R), E out (phase C, group 0)                     */
-constexpr size_t SMEM_BYTES = (size_t)(4 * BUF + REGA + REGB + 16 * TT) * sizeof(float2) + (size_t)16 * TT * sizeof(float4);
-constexpr size_t Z512_OFF = (size_t)128 * 256 * 16;   /* float2 offset of Z512[512] inside the Z buffer                   */
-constexpr size_t ZX_ELEMS = Z512_OFF + 512;           /* float2 in the Z buffer (fits one half-spectrum array)            */
-constexpr size_t EX_ELEMS = (size_t)128 * 128 * 16;   /* float2 in the E buffer                                           */
+constexpr size_t SMEM_BYTES = (size_t)(4 * BUF + REGA + REGB + 16 * TT) * sizeof(float2) + (size_t)16 * TT * sizeof(float4) + 16;
+constexpr size_t Z512_OFF = (size_t)128 * 256 * 16;   /* float2 offset of Z512[512] inside the Z array (fits one half-spectrum array) */
+constexpr int NARRIVE = 2 * NCTA;                     /* every group of every CTA arrives at every grid barrier           */
 
 struct Args {
   float2 *state;
-  float2 *Zx, *Ex;               /* exchange buffers; a prologue launch finds every word tagged with the parity of step0 - 1 */
-  unsigned long long *w512;      /* progress of column 512: local steps whose Z512 block CTA 128 has consumed; zero at launch */
+  float2 *Eg;
+  float2 *Zg;
   const float2 *tw;              /* tw[j] = exp(-2 pi i j / 1024) */
+  unsigned long long *bar;       /* bar[0]: counter of barrier A (Z complete), bar[16]: barrier B (E complete); zero at launch */
   long long nsteps;
   unsigned long long step0;
   int prologue;                  /* 1: E is stale (after pss_set_field): rebuild it from the state first */
+  int prio;                      /* 1: in phase C group 1 waits for group 0's transforms (PSS_P2D_PRIO=0 disables) */
+  int gate;                      /* 1: the noise warps pause while their group computes (PSS_NOISE_GATE=0 disables) */
   int dbg;                       /* timing experiments only (-DPSS_P2D_DEBUG): 1 = skip the transforms, 2 = skip the noise */
   long long *ts;                 /* timing experiments only (-DPSS_P2D_DEBUG): globaltimer stamps [cta][group][32] of the last-but-one step */
 };
@@ -208,65 +206,47 @@ __device__ __forceinline__ void fwd_dit(float2 (&v)[16], const Lane &ln) {
 /* all 256 transform threads */
 __device__ __forceinline__ void tsync_all() { asm volatile("bar.sync 7, 256;" ::: "memory"); }
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
-
-/* ---- flag-in-data exchange: relaxed gpu-scope 16-byte accesses (L2; never the L1) ---- */
-__device__ __forceinline__ uint4 ld_relaxed16(const void *p) {
-  uint4 r;
-  asm volatile("ld.relaxed.gpu.global.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p) : "memory");
-  return r;
-}
-__device__ __forceinline__ void st_relaxed16(void *p, uint4 v) {
-  asm volatile("st.relaxed.gpu.global.v4.u32 [%0], {%1, %2, %3, %4};" ::"l"(p), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
-}
-__device__ __forceinline__ uint2 ld_relaxed8(const void *p) {
-  uint2 r;
-  asm volatile("ld.relaxed.gpu.global.v2.u32 {%0, %1}, [%2];" : "=r"(r.x), "=r"(r.y) : "l"(p) : "memory");
-  return r;
-}
-__device__ __forceinline__ void st_relaxed8(void *p, uint2 v) {
-  asm volatile("st.relaxed.gpu.global.v2.u32 [%0], {%1, %2};" ::"l"(p), "r"(v.x), "r"(v.y) : "memory");
-}
-/* every word carries the parity `tag` in its least significant bit */
-__device__ __forceinline__ bool all_tagged(uint4 r, uint32_t tag) {
-  return tag ? (((r.x & r.y & r.z & r.w) & 1u) != 0u) : (((r.x | r.y | r.z | r.w) & 1u) == 0u);
-}
-__device__ __forceinline__ uint32_t tagw(uint32_t w, uint32_t tag) { return (w & ~1u) | tag; }
-__device__ __forceinline__ uint4 tag4(uint4 r, uint32_t tag) { return make_uint4(tagw(r.x, tag), tagw(r.y, tag), tagw(r.z, tag), tagw(r.w, tag)); }
-/* fail the launch instead of hanging the GPU: wall clock, 30 s */
-__device__ __forceinline__ void watchdog(unsigned &spins, unsigned long long &t0) {
-  if (((++spins) & 0xfffu) == 0) {
-    unsigned long long t;
-    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
-    if (t0 == 0) t0 = t;
-    else if (t - t0 > 30000000000ull) __trap();
-  }
+__device__ __forceinline__ void st_cg16(void *p, uint4 v) {
+  asm volatile("st.global.cg.v4.u32 [%0], {%1, %2, %3, %4};" ::"l"(p), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
 }
 
-/* The CTA's contiguous input block (NP x 256 x 16 bytes) -> staging tile, by all 256 transform threads: every thread
- * polls its NP pieces until every word carries the parity of this step (in registers: the other group may still be
- * reading the staging tile), then the CTA synchronises, the pieces go to shared memory and the CTA synchronises again. */
-template <int NP> __device__ __forceinline__ void poll_tile(float2 *dst, const float2 *src, int tid, uint32_t tag) {
-  const char *sp = reinterpret_cast<const char *>(src) + tid * 16;
-  uint4 *d = reinterpret_cast<uint4 *>(dst) + tid;
-  uint4 r[NP];
-  unsigned pend = (1u << NP) - 1u, spins = 0;
-  unsigned long long t0 = 0;
-#pragma unroll
-  for (int i = 0; i < NP; ++i) r[i] = ld_relaxed16(sp + i * 4096);
+/* ---- grid barrier: one monotonically increasing counter per barrier kind, zeroed by the host before the launch.
+ * A group arrives with a release reduction by one thread after its own bar.sync (the group's global stores
+ * happen-before it through the CTA barrier).  Only thread 0 of a CTA polls (acquire loads); everybody else waits at a
+ * CTA barrier for it, then fetches the block. ---- */
+__device__ __forceinline__ void grid_arrive(unsigned long long *ctr) {
+  asm volatile("red.release.gpu.global.add.u64 [%0], 1;" ::"l"(ctr) : "memory");
+}
+/* arrival of a group that wrote nothing the other CTAs read (it only reports that its input block has been fetched:
+ * the asynchronous copies were waited for, so no fence is needed) */
+__device__ __forceinline__ void grid_arrive_relaxed(unsigned long long *ctr) {
+  asm volatile("red.relaxed.gpu.global.add.u64 [%0], 1;" ::"l"(ctr) : "memory");
+}
+__device__ __forceinline__ void grid_poll(const unsigned long long *ctr, unsigned long long target) {
+  unsigned long long v, t0 = 0;
+  unsigned spins = 0;
   for (;;) {
-#pragma unroll
-    for (int i = 0; i < NP; ++i)
-      if (((pend >> i) & 1u) && all_tagged(r[i], tag)) pend &= ~(1u << i);
-    if (pend == 0) break;
-    watchdog(spins, t0);
-#pragma unroll
-    for (int i = 0; i < NP; ++i)
-      if ((pend >> i) & 1u) r[i] = ld_relaxed16(sp + i * 4096);
+    asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(ctr) : "memory");
+    if (v >= target) break;
+    if (((++spins) & 0x3fffu) == 0) { /* watchdog on the wall clock (30 s): fail the launch instead of hanging the GPU */
+      unsigned long long t;
+      asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+      if (t0 == 0) t0 = t;
+      else if (t - t0 > 30000000000ull) __trap();
+    }
   }
-  tsync_all();
+}
+/* 16 bytes global (L2) -> shared, asynchronous, no register staging */
+__device__ __forceinline__ void cp_async16(uint32_t dst, const void *src) {
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
+}
+/* the CTA's contiguous input block (N16 x 256 x 16 bytes) into a staging tile, all 256 transform threads */
+template <int N16> __device__ __forceinline__ void load_block(float2 *dst, const float2 *src, int tid) {
+  const uint32_t d = smem_u32(dst) + tid * 16;
+  const char *sp = reinterpret_cast<const char *>(src) + tid * 16;
 #pragma unroll
-  for (int i = 0; i < NP; ++i) d[i * 256] = r[i];
-  tsync_all();
+  for (int i = 0; i < N16; ++i) cp_async16(d + i * 4096, sp + i * 4096);
+  asm volatile("cp.async.wait_all;" ::: "memory");
 }
 
 /* ------------------------------------------------------------------------------------------ */
@@ -277,6 +257,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_persist2d(const __grid_constant_
   float2 *regB = regA + REGA;                                   /* staging B                               */
   float2 *zbuf = regB + REGB;                                   /* [16 r][256 tid] unit noise z            */
   float4 *tab = reinterpret_cast<float4 *>(zbuf + 16 * TT);     /* [16 r][256 tid] per-mode coefficients   */
+  volatile int *hold = reinterpret_cast<volatile int *>(tab + 16 * TT); /* [2]: group g is computing: its noise warps pause */
 
   const int tid = threadIdx.x & (TT - 1);
   const bool noisew = threadIdx.x >= TT;
@@ -293,6 +274,9 @@ __global__ void __launch_bounds__(THREADS, 1) k_persist2d(const __grid_constant_
   const bool noisy = D0.noisy != 0;
   const long long nphase = A.nsteps + (A.prologue ? 1 : 0);
 
+  if (threadIdx.x < 2) hold[threadIdx.x] = 0;
+  __syncthreads();
+
   if (noisew) {
     asm volatile("setmaxnreg.dec.sync.aligned.u32 64;"); /* hand registers to the transform warps */
     /* ============ noise warps: z(step s+1) is drawn while the transform warps work on step s ============ */
@@ -308,9 +292,14 @@ __global__ void __launch_bounds__(THREADS, 1) k_persist2d(const __grid_constant_
       if (s >= 1) nb_sync(5 + g); /* the group has consumed z(s-1) */
       if (colw && !P2D_DBG(1)) {
         float2 *zw = zbuf + tid;
-#pragma unroll 2
-        for (int r = 0; r < 16; ++r)
+#pragma unroll 1
+        for (int r = 0; r < 16; r += 2) {
+          /* pause while the group's transform warps compute; they clear the flag when they wait (exchange in flight,
+           * or z itself needed) */
+          if (A.gate) while (hold[g]) __nanosleep(200);
           zw[r * TT] = noise_mode(K, kx, kyb + 16 * (r & 3) + 256 * (r >> 2), selfc);
+          zw[(r + 1) * TT] = noise_mode(K, kx, kyb + 16 * ((r + 1) & 3) + 256 * ((r + 1) >> 2), selfc);
+        }
       }
       nb_arrive(3 + g);
     }
@@ -381,25 +370,26 @@ __global__ void __launch_bounds__(THREADS, 1) k_persist2d(const __grid_constant_
   const int es0 = (tq >> 2) * 16 + eidx(tq & 3, L, b, tq >> 2);                  /* E scatter, direct: + 256 a   */
   const int es1 = (tq >> 2) * 16 + eidx(tq & 3, 2 + L, b, tq >> 2);              /* mirror                       */
   const int gt = tid & (GT - 1), cq = gt & 7;                                    /* copy-out: lane cq of chunk (gt >> 3) + 16 i */
+  unsigned long long *ctrA = A.bar, *ctrB = A.bar + 16;
+  unsigned long long nA = 0, nB = 0;   /* barriers of each kind this thread has been through */
+  gsync(g);
+
+  /* first phase R of a launch that finds E valid: no barrier to wait for */
+  if (!A.prologue && roww && nphase > 0) {
+    load_block<4>(regB, A.Eg + (size_t)b * 2048, tid);
+    tsync_all();
+  }
 
   float2 v[16];
 #pragma unroll 1
   for (long long it = 0; it < nphase; ++it) {
     const bool pro = A.prologue && it == 0;
     const long long ls = it - (A.prologue ? 1 : 0);
-    /* parity tags: Z produced and consumed by step s and the E it consumes carry s & 1; the E written in step s is
-     * consumed by step s + 1; the prologue writes the E of step step0 */
-    const unsigned long long sabs = A.step0 + (unsigned long long)(ls < 0 ? 0 : ls);
-    const uint32_t tag = (uint32_t)(sabs & 1ull), tagE = pro ? tag : (tag ^ 1u);
     if (!pro) {
       /* ======================= phase R: inverse-x of E, product, forward-x -> Z ======================= */
       if (roww) {
+        if (gt == 0) hold[g] = 1;
         TS(0);
-        poll_tile<4>(regB, A.Ex + (size_t)b * 2048, tid, tag);
-        TS(1);
-        /* column 512 feeds nothing back: before this line overwrites its slot, CTA 128 must have consumed step ls - 1 */
-        unsigned long long w512 = 0;
-        if (tq == 0) asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(w512) : "l"(A.w512) : "memory");
         /* D_spec input, conjugated (inverse transform = conj o forward o conj); only |k| < 256 is non-zero:
          * k3 = 0 reads column kx = k00 + 16 j (chunk +8 per j), k3 = 3 the mirror slot of kx = 256 - k00 - 16 j */
 #pragma unroll
@@ -432,12 +422,8 @@ __global__ void __launch_bounds__(THREADS, 1) k_persist2d(const __grid_constant_
           zout[zs0 + 128 * j] = v[j];
           zout[zs1 + 128 * j] = v[j + 4];
           if (j == 0 && tq == 0) {
-            unsigned spins = 0;
-            unsigned long long t0 = 0;
-            while (w512 < (unsigned long long)ls) { watchdog(spins, t0); asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(w512) : "l"(A.w512) : "memory"); }
-            st_relaxed8(A.Zx + Z512_OFF + 2 * bg + L, make_uint2(tagw(__float_as_uint(v[8].x), tag), tagw(__float_as_uint(v[8].y), tag))); /* k = 512 */
+            A.Zg[Z512_OFF + 2 * bg + L] = v[8];                      /* k = 512: column 512 itself          */
             zout[zidx(1, L, 2, 0, bg)] = v[12];                      /* k = 768: mirror of kx = 256 (group 1 of CTA 0) */
-            zout[zidx(0, L, 2, 0, bg)] = make_float2(0.f, 0.f);      /* the unused mirror slot of kx = 0 is tagged like the rest */
           } else {
             zout[zs2 - 128 * j] = v[j + 8];
             zout[zs3 - 128 * j] = v[j + 12];
@@ -445,25 +431,38 @@ __global__ void __launch_bounds__(THREADS, 1) k_persist2d(const __grid_constant_
         }
         gsync(g);
         TS(4);
-        /* copy-out: 128 chunks of 128 bytes, 8 lanes per chunk, whole lines; the store IS the signal */
+        /* copy-out: 128 chunks of 128 bytes, 8 lanes per chunk, whole lines */
         {
           const uint4 *src = reinterpret_cast<const uint4 *>(zout);
-          uint4 *dst = reinterpret_cast<uint4 *>(A.Zx);
+          uint4 *dst = reinterpret_cast<uint4 *>(A.Zg);
 #pragma unroll
           for (int i = 0; i < 8; ++i) {
             const int c = (gt >> 3) + 16 * i;
-            st_relaxed16(dst + ((size_t)c * 256 + bg) * 8 + cq, tag4(src[c * 8 + cq], tag));
+            st_cg16(dst + ((size_t)c * 256 + bg) * 8 + cq, src[c * 8 + cq]);
           }
         }
         TS(5);
       }
-      /* ======================= phase C: forward-y of Z, Eq. 15/16/18, inverse-y -> E ======================= */
-      if (roww) poll_tile<8>(regA, A.Zx + (size_t)b * 4096, tid, tag);
-      else {
-        poll_tile<1>(regA, A.Zx + Z512_OFF, tid, tag);
-        if (tid == 0) asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(A.w512), "l"((unsigned long long)(ls + 1)) : "memory");
+      gsync(g);
+      if (gt == 0) {
+        hold[g] = 0;
+        if (roww) grid_arrive(ctrA);
+        else grid_arrive_relaxed(ctrA);
       }
+      nA += 1;
+      TS(6);
+      /* ======================= phase C: forward-y of Z, Eq. 15/16/18, inverse-y -> E ======================= */
+      if (tid == 0) grid_poll(ctrA, nA * NARRIVE);
+      tsync_all();
+      TS(7);
+      if (roww) load_block<8>(regA, A.Zg + (size_t)b * 4096, tid);
+      else load_block<1>(regA, A.Zg + Z512_OFF, tid);
+      tsync_all();
       TS(8);
+      /* the kept columns are the critical path (their inverse transform feeds the next exchange): group 1 starts its
+       * forward transform when group 0 has finished both of its own, and runs while barrier B is in flight */
+      if (roww && g == 1 && A.prio) asm volatile("bar.sync 8, 256;" ::: "memory");
+      if (gt == 0) hold[g] = 1;
       if (colw) {
 #pragma unroll
         for (int a = 0; a < 8; ++a) {
@@ -482,10 +481,18 @@ __global__ void __launch_bounds__(THREADS, 1) k_persist2d(const __grid_constant_
 #pragma unroll
         for (int a = 0; a < 16; ++a) v[a] = make_float2(0.f, 0.f);
       }
+      if (!kept) { /* nothing of this group feeds E: arrive as soon as the input tile has been consumed */
+        gsync(g);
+        if (gt == 0) grid_arrive_relaxed(ctrB);
+      }
       if (!P2D_DBG(0)) fwd_dif(v, ln);
       TS(10);
       /* v[r] = P_q at ky(r): Eq. 15 + Eq. 16 + Eq. 18, then the next factor's (conjugated) input */
-      if (noisy) nb_sync(3 + g);
+      if (noisy) {
+        if (gt == 0) hold[g] = 0;      /* z is needed now: let the noise warps finish */
+        nb_sync(3 + g);
+        if (gt == 0 && kept) hold[g] = 1;
+      }
 #pragma unroll
       for (int r = 0; r < 16; ++r) {
         const float4 tt = tab[r * TT + tid];
@@ -497,17 +504,24 @@ __global__ void __launch_bounds__(THREADS, 1) k_persist2d(const __grid_constant_
         v[r] = make_float2(st[r].x * tt.w, -st[r].y * tt.w);
       }
       if (noisy && ls + 1 < A.nsteps) nb_arrive(5 + g);
+      if (!noisy && gt == 0 && !kept) hold[g] = 0;
       TS(11);
       /* no barrier before fwd_dit: its first pass writes the 16 slots this thread read last in fwd_dif */
-    } else if (kept) {
+    } else {
+      if (kept) {
 #pragma unroll
-      for (int r = 0; r < 16; ++r) {
-        const float fc = tab[r * TT + tid].w;
-        v[r] = make_float2(st[r].x * fc, -st[r].y * fc);
+        for (int r = 0; r < 16; ++r) {
+          const float fc = tab[r * TT + tid].w;
+          v[r] = make_float2(st[r].x * fc, -st[r].y * fc);
+        }
+      } else {
+        gsync(g);
+        if (gt == 0) grid_arrive_relaxed(ctrB);
       }
     }
     if (kept) {
       if (!P2D_DBG(0)) fwd_dit(v, ln);
+      if (!pro && A.prio) asm volatile("bar.arrive 8, 256;" ::: "memory");
       TS(12);
       /* conj(v[a]) = psi_x[kx][y = 64 a + tq]; pack rows y (A) and y + 512 (B); chunk per consumer CTA p >> 2 */
 #pragma unroll
@@ -516,7 +530,6 @@ __global__ void __launch_bounds__(THREADS, 1) k_persist2d(const __grid_constant_
         const float2 bv = make_float2(v[a + 8].x, -v[a + 8].y);
         if (selfc) {
           regB[es0 + 256 * a] = make_float2(av.x, bv.x);                       /* the C2R keeps the real part there */
-          regB[es1 + 256 * a] = make_float2(0.f, 0.f);                         /* unused mirror slot                */
         } else {
           regB[es0 + 256 * a] = make_float2(av.x - bv.y, av.y + bv.x);          /* A + iB              */
           regB[es1 + 256 * a] = make_float2(av.x + bv.y, bv.x - av.y);          /* conj(A) + i conj(B) */
@@ -526,14 +539,27 @@ __global__ void __launch_bounds__(THREADS, 1) k_persist2d(const __grid_constant_
       TS(13);
       {
         const uint4 *src = reinterpret_cast<const uint4 *>(regB);
-        uint4 *dst = reinterpret_cast<uint4 *>(A.Ex);
+        uint4 *dst = reinterpret_cast<uint4 *>(A.Eg);
 #pragma unroll
         for (int i = 0; i < 8; ++i) {
           const int bp = (gt >> 3) + 16 * i;
-          st_relaxed16(dst + ((size_t)bp * 128 + b) * 8 + cq, tag4(src[bp * 8 + cq], tagE));
+          st_cg16(dst + ((size_t)bp * 128 + b) * 8 + cq, src[bp * 8 + cq]);
         }
       }
       TS(14);
+      gsync(g);
+      if (gt == 0) { hold[g] = 0; grid_arrive(ctrB); }
+      TS(15);
+    }
+    nB += 1;
+    /* entry of the next phase R: the CTA's E block (16 KB) as soon as barrier B is open */
+    if (it + 1 < nphase && roww) {
+      if (tid == 0) grid_poll(ctrB, nB * NARRIVE);
+      tsync_all();
+      TS(16);
+      load_block<4>(regB, A.Eg + (size_t)b * 2048, tid);
+      tsync_all();
+      TS(17);
     }
   }
 
@@ -541,11 +567,6 @@ __global__ void __launch_bounds__(THREADS, 1) k_persist2d(const __grid_constant_
 #pragma unroll
     for (int r = 0; r < 16; ++r) A.state[(size_t)kx * N + kyb + 16 * (r & 3) + 256 * (r >> 2)] = st[r];
   }
-}
-
-/* every word of an exchange buffer gets the parity `lsb` (host side, before a prologue launch) */
-__global__ void k_fill_tag(uint32_t *p, size_t n, uint32_t lsb) {
-  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) p[i] = lsb;
 }
 
 }  // namespace p2d
