@@ -181,10 +181,13 @@ static void philox4x32_10(const uint32_t c_in[4], const uint32_t k_in[2], uint32
  * ("intermediate") fields defined as operators applied to other fields, a list of rhs terms.
  * ------------------------------------------------------------------------------------------ */
 struct Def { opss_op op; int src; };
+struct ATerm { opss_op outer; std::vector<int> factors; };
 struct Field {
   std::string name;
   bool dynamic;
   std::vector<Def> defs;      /* aux only: psi_q = sum coef Op(q) src_q          */
+  std::vector<opss_op> alhs;  /* aux only: its own lhs, den(q) psi_q = rhs; empty = the bare field */
+  std::vector<ATerm> aterms;  /* aux only: rhs terms that are products of fields                  */
   std::vector<opss_op> lhs;   /* dynamic only: dt phi + sum coef Op(q) phi = rhs */
   bool noisy; double D; int qpow;
   std::vector<cplx> hat;      /* half-spectrum, unnormalised forward DFT         */
@@ -267,6 +270,13 @@ static int max_order(const opss_system *s, int f) {
     for (int g : t.factors)
       if (g == f && (int)t.factors.size() > nmax) nmax = (int)t.factors.size();
   }
+  /* products that define intermediate fields count as well ("fields that form part of nonlinearities") */
+  for (const Field &F : s->fields)
+    for (const ATerm &t : F.aterms) {
+      if (t.factors.size() < 2) continue;
+      for (int g : t.factors)
+        if (g == f && (int)t.factors.size() > nmax) nmax = (int)t.factors.size();
+    }
   return nmax;
 }
 
@@ -360,6 +370,20 @@ static void one_step(opss_system *s) {
   const int nth = s->nthreads;
   const int nf = (int)s->fields.size();
 
+  /* de-aliased copy of field f in real space, made once its spectrum is final for this step */
+  std::vector<std::vector<double>> real(nf);
+  auto to_real = [&](int f) {
+    if (!real[f].empty()) return;
+    const int order = max_order(s, f);
+    std::vector<cplx> masked(s->fields[f].hat);
+#pragma omp parallel for num_threads(nth) schedule(static)
+    for (int64_t m = 0; m < M; ++m) {
+      int64_t k[3]; mode_of(d, m, k);
+      if (!keep_mode(s, order, k)) masked[m] = cplx(0, 0);
+    }
+    c2r(masked, real[f], d, nth);
+  };
+
   /* 1. intermediate fields psi_k, creation order, from time-t values (A12) */
   for (int a = 0; a < nf; ++a) {
     Field &fa = s->fields[a];
@@ -373,20 +397,40 @@ static void one_step(opss_system *s) {
         fa.hat[m] += op_eval(s, df.op, k) * src[m];
       }
     }
+    /* rhs terms that are products: the factors (dynamic or earlier intermediate fields) are final */
+    for (const ATerm &t : fa.aterms) {
+      std::vector<double> P(NS, 1.0);
+      for (int g : t.factors) {
+        to_real(g);
+        const std::vector<double> &r = real[g];
+#pragma omp parallel for num_threads(nth) schedule(static)
+        for (int64_t x = 0; x < NS; ++x) P[x] *= r[x];
+      }
+      std::vector<cplx> Ph;
+      r2c(P, Ph, d, nth);
+#pragma omp parallel for num_threads(nth) schedule(static)
+      for (int64_t m = 0; m < M; ++m) {
+        int64_t k[3]; mode_of(d, m, k);
+        fa.hat[m] += op_eval(s, t.outer, k) * Ph[m];
+      }
+    }
+    /* its own lhs: den(q) psi_q = rhs_q, psi_q = 0 where den(q) = 0 (as 1/q at q = 0, A10) */
+    if (!fa.alhs.empty()) {
+#pragma omp parallel for num_threads(nth) schedule(static)
+      for (int64_t m = 0; m < M; ++m) {
+        int64_t k[3]; mode_of(d, m, k);
+        cplx den(0, 0);
+        for (const opss_op &o : fa.alhs) den += op_eval(s, o, k);
+        fa.hat[m] = (den == cplx(0, 0)) ? cplx(0, 0) : fa.hat[m] / den;
+      }
+    }
   }
 
   /* 2.+3. de-aliased copies of the factor fields, to real space */
-  std::vector<std::vector<double>> real(nf);
   for (int f = 0; f < nf; ++f) {
     const int order = max_order(s, f);
     if (order < 2) continue;
-    std::vector<cplx> masked(s->fields[f].hat);
-#pragma omp parallel for num_threads(nth) schedule(static)
-    for (int64_t m = 0; m < M; ++m) {
-      int64_t k[3]; mode_of(d, m, k);
-      if (!keep_mode(s, order, k)) masked[m] = cplx(0, 0);
-    }
-    c2r(masked, real[f], d, nth);
+    to_real(f);
   }
 
   /* 3.+4.+5a. N_i(q) = sum_t outer_t(q) F[prod factors](q)  + explicit linear terms (Eq. 15) */
@@ -502,6 +546,33 @@ int opss_add_aux_def(opss_system *s, int aux, const opss_op *op, int src) {
   return OPSS_OK;
 }
 
+int opss_add_aux_lhs(opss_system *s, int aux, const opss_op *op) {
+  if (!s) return OPSS_EINVAL;
+  if (s->finalized) return OPSS_ESTATE;
+  if (!fid_ok(s, aux) || !op_ok(s, op)) return OPSS_EINVAL;
+  if (s->fields[aux].dynamic) return OPSS_EINVAL;
+  s->fields[aux].alhs.push_back(*op);
+  return OPSS_OK;
+}
+
+int opss_add_aux_term(opss_system *s, int aux, const opss_op *outer, int nfactors, const int *factor_fields) {
+  if (!s) return OPSS_EINVAL;
+  if (s->finalized) return OPSS_ESTATE;
+  if (!fid_ok(s, aux) || !op_ok(s, outer) || !factor_fields) return OPSS_EINVAL;
+  if (s->fields[aux].dynamic) return OPSS_EINVAL;
+  if (nfactors < 2) return OPSS_EINVAL; /* one factor is opss_add_aux_def */
+  if (nfactors > 4) return OPSS_EUNSUPPORTED;
+  ATerm t; t.outer = *outer;
+  for (int i = 0; i < nfactors; ++i) {
+    const int g = factor_fields[i];
+    if (!fid_ok(s, g)) return OPSS_EINVAL;
+    if (!s->fields[g].dynamic && g >= aux) return OPSS_EINVAL; /* dynamic or EARLIER intermediate fields only (A12) */
+    t.factors.push_back(g);
+  }
+  s->fields[aux].aterms.push_back(t);
+  return OPSS_OK;
+}
+
 int opss_add_term(opss_system *s, int field, const opss_op *outer, int nfactors,
                   const int *factor_fields) {
   if (!s) return OPSS_EINVAL;
@@ -545,7 +616,7 @@ int opss_finalize(opss_system *s, size_t *workspace_bytes) {
   for (const Field &f : s->fields) ndyn += f.dynamic ? 1 : 0;
   if (ndyn == 0) return OPSS_EINVAL;
   for (size_t a = 0; a < s->fields.size(); ++a)
-    if (!s->fields[a].dynamic && s->fields[a].defs.empty()) return OPSS_EINVAL; /* undefined aux */
+    if (!s->fields[a].dynamic && s->fields[a].defs.empty() && s->fields[a].aterms.empty()) return OPSS_EINVAL; /* undefined aux */
   for (Field &f : s->fields) f.hat.assign(s->d.nmodes(), cplx(0, 0));
   s->finalized = true;
   if (workspace_bytes) *workspace_bytes = 0; /* the oracle owns its memory */

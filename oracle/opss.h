@@ -47,6 +47,12 @@ int opss_create(opss_system **out, int ndim, const int64_t n[3], const double dx
 int opss_add_field(opss_system *, const char *name, int dynamic, int *field_id);
 int opss_add_linear(opss_system *, int field, const opss_op *op);
 int opss_add_aux_def(opss_system *, int aux, const opss_op *op, int src);
+/* intermediate field with its own lhs: (sum of the ops added here)(q) * psi_q = rhs_q; psi_q = 0 where
+ * the sum vanishes.  None added = the bare field. */
+int opss_add_aux_lhs(opss_system *, int aux, const opss_op *op);
+/* rhs term of an intermediate field that is a product of >= 2 fields: psi_q += outer(q) F[prod](q);
+ * factors: dynamic fields or intermediate fields created earlier. */
+int opss_add_aux_term(opss_system *, int aux, const opss_op *outer, int nfactors, const int *factor_fields);
 int opss_add_term(opss_system *, int field, const opss_op *outer, int nfactors,
                   const int *factor_fields);
 int opss_set_noise(opss_system *, int field, double D, int q_power);

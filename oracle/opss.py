@@ -48,6 +48,8 @@ def lib():
         L.opss_add_linear.argtypes = [P, C.c_int, C.POINTER(_Op)]
         L.opss_add_aux_def.argtypes = [P, C.c_int, C.POINTER(_Op), C.c_int]
         L.opss_add_term.argtypes = [P, C.c_int, C.POINTER(_Op), C.c_int, C.POINTER(C.c_int)]
+        L.opss_add_aux_lhs.argtypes = [P, C.c_int, C.POINTER(_Op)]
+        L.opss_add_aux_term.argtypes = [P, C.c_int, C.POINTER(_Op), C.c_int, C.POINTER(C.c_int)]
         L.opss_set_noise.argtypes = [P, C.c_int, C.c_double, C.c_int]
         L.opss_set_dealias.argtypes = [P, C.c_int]
         L.opss_finalize.argtypes = [P, C.POINTER(C.c_size_t)]
@@ -127,6 +129,14 @@ class System:
 
     def add_aux_def(self, aux, op, src):
         _chk(lib().opss_add_aux_def(self._h, int(aux), C.byref(_op(op)), int(src)))
+
+    def add_aux_lhs(self, aux, op):
+        _chk(lib().opss_add_aux_lhs(self._h, int(aux), C.byref(_op(op))))
+
+    def add_aux_term(self, aux, outer, factors):
+        factors = [int(f) for f in factors]
+        arr = (C.c_int * max(1, len(factors)))(*factors)
+        _chk(lib().opss_add_aux_term(self._h, int(aux), C.byref(_op(outer)), len(factors), arr))
 
     def add_term(self, field, outer, factors):
         factors = [int(f) for f in factors]

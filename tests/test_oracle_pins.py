@@ -624,3 +624,87 @@ def test_oracle_error_codes(oracle):
     with pytest.raises(oracle.OracleError) as e:
         s.add_field("late", True)
     assert e.value.code == oracle.ESTATE
+
+
+# ------------------------------------------------------------------------------------------ P15, P16
+@pytest.mark.parametrize("n,dx", [((16,), (0.7,)), ((8, 16), (1.0, 0.5)), ((4, 8, 8), (1.0, 2.0, 0.5))])
+def test_p15_intermediate_field_with_its_own_lhs(oracle, n, dx):
+    """"psi + psi*q^2 = -q^2 phi"  <=>  psi_q = -q^2 (1 + q^2)^-1 phi_q, mode by mode.  The
+    intermediate field is observed through an explicit linear term dt u = psi: u_q(1) - u_q(0) = dt psi_q.  Also an
+    lhs that vanishes at q = 0 ("q^2 psi = phi", a Poisson solve): psi_0 = 0 (reading A10)."""
+    dt = 0.25
+    rng = np.random.default_rng(15)
+    phi0 = rng.standard_normal(n[::-1])
+    qs = []
+    for j in range(len(n)):
+        k = np.arange(n[j] // 2 + 1) if j == 0 else np.fft.fftfreq(n[j], 1.0 / n[j])
+        qs.append(2 * np.pi * np.abs(k) / (n[j] * dx[j]))
+    q2 = sum(g * g for g in np.meshgrid(*qs[::-1], indexing="ij"))
+    for lhs, num, expect in (
+            ([{"coef": 1.0}, {"coef": 1.0, "q2_pow": 1}], {"coef": -1.0, "q2_pow": 1}, lambda: -q2 / (1.0 + q2)),
+            ([{"coef": 1.0, "q2_pow": 1}], {"coef": 1.0}, lambda: np.where(q2 > 0, 1.0 / np.where(q2 > 0, q2, 1.0), 0.0)),
+            ([{"coef": 2.0}], {"coef": 3.0, "q2_pow": 2}, lambda: 1.5 * q2 * q2)):
+        s = oracle.System(n, dx, dt, prec="f64", seed=3)
+        phi = s.add_field("phi", True)
+        u = s.add_field("u", True)
+        psi = s.add_field("psi", False)
+        for o in lhs:
+            s.add_aux_lhs(psi, o)
+        s.add_aux_def(psi, num, phi)
+        s.add_term(u, {"coef": 1.0}, [psi])
+        s.finalize()
+        s.set_field(phi, phi0)
+        s.set_field(u, np.zeros(n[::-1]))
+        ph = s.get_field_fourier_f64(phi)
+        s.step(1)
+        got = s.get_field_fourier_f64(u) / dt
+        want = expect() * ph
+        assert np.abs(got - want).max() <= 1e-12 * max(1.0, np.abs(want).max())
+        assert np.array_equal(s.get_field_fourier_f64(phi), ph)          # a field without an equation does not move
+
+
+@pytest.mark.parametrize("n", [8, 16])
+def test_p16_two_level_product_is_the_nested_direct_convolution(oracle, n):
+    """an intermediate field that is itself a product, mu = phi*phi, used in dt u = -q^2 (mu*phi).
+    Both products are quadratic, so every factor copy is truncated at |s(k)| < N/3; expected value:
+    the two nested O(N^2) NON-wrapping convolutions of Eq. 5 written out with the masks, and with no mask the circular ones."""
+    rng = np.random.default_rng(100 + n)
+    phi0 = rng.standard_normal(n)
+    full = np.fft.fft(phi0)
+    dt = 0.5
+    for dealias in (oracle.DEALIAS_OFF, oracle.DEALIAS_PAPER):
+        s = oracle.System((n,), (1.0,), dt, prec="f64", seed=1)
+        phi = s.add_field("phi", True)
+        u = s.add_field("u", True)
+        mu = s.add_field("mu", False)
+        s.add_aux_term(mu, {"coef": 1.0}, [phi, phi])
+        s.add_term(u, {"coef": -1.0, "q2_pow": 1}, [mu, phi])
+        s.set_dealias(dealias)
+        s.finalize()
+        s.set_field(phi, phi0)
+        s.set_field(u, np.zeros(n))
+        s.step(1)
+        got = s.get_field_fourier_f64(u) / dt
+        keep = [k for k in range(n) if dealias == oracle.DEALIAS_OFF or 3 * abs(_signed(k, n)) < n]
+        wrap = dealias == oracle.DEALIAS_OFF
+        muh = np.zeros(n, dtype=complex)
+        for q in range(n):
+            for k in keep:
+                for l in keep:
+                    if (wrap and (k + l - q) % n == 0) or (not wrap and _signed(k, n) + _signed(l, n) == _signed(q, n)):
+                        muh[q] += full[k] * full[l] / n
+        if not wrap:   # sums outside (-N/2, N/2] do not exist without wrapping: |k + l| < 2N/3 can exceed N/2 -> they alias
+            muh = np.zeros(n, dtype=complex)
+            for k in keep:
+                for l in keep:
+                    muh[(k + l) % n] += full[k] * full[l] / n   # what the lattice really holds (aliased outside the kept band)
+        for q in range(n // 2 + 1):
+            if not wrap and 3 * abs(_signed(q, n)) >= n:
+                continue
+            acc = 0j
+            for k in keep:      # mu is a factor of a quadratic product: its copy is truncated too
+                for l in keep:
+                    if (wrap and (k + l - q) % n == 0) or (not wrap and _signed(k, n) + _signed(l, n) == _signed(q, n)):
+                        acc += muh[k] * full[l] / n
+            q2 = (2 * np.pi * q / n) ** 2
+            assert abs(got[q] - (-q2) * acc) <= 1e-11 * max(1.0, abs(acc)), (dealias, q)
