@@ -74,6 +74,16 @@ int pss_add_linear(pss_system *, int field, const pss_op *op);
 /* intermediate field definition psi_q += coef*Op(q)*src_q; src is a dynamic
  * field or an EARLIER aux field. */
 int pss_add_aux_def(pss_system *, int aux, const pss_op *op, int src);
+/* Intermediate field with its own lhs ("psi + psi*q^2 = -q^2*phi"): den(q) psi_q = rhs_q with
+ * den(q) = sum of the operators added here; psi_q = 0 where den(q) = 0 (reading A10).  None added = the bare field.
+ * The CUDA path takes real-valued lhs operators (even total derivative order) and at most two such fields
+ * (PSS_EUNSUPPORTED at pss_finalize otherwise). */
+int pss_add_aux_lhs(pss_system *, int aux, const pss_op *op);
+/* rhs term of an intermediate field that is a PRODUCT of 2..4 fields: psi_q += outer(q) F[prod](q).
+ * factor_fields: host array of dynamic fields or intermediate fields created earlier.  Such a field is re-evaluated
+ * every step in its own round of the two step kernels (one round per dependency level) before the fields that use it;
+ * 2D/3D single systems (PSS_EUNSUPPORTED for 1D or ensembles). */
+int pss_add_aux_term(pss_system *, int aux, const pss_op *outer, int nfactors, const int *factor_fields);
 /* rhs term (Eq. 15): N_q += outer(q) * F[ prod_k factor_k(x) ].  nfactors == 1 is an
  * explicit linear term evaluated in Fourier space (no transform, no mask).  factor_fields: host array. */
 int pss_add_term(pss_system *, int field, const pss_op *outer, int nfactors, const int *factor_fields);

@@ -20,10 +20,15 @@ def needs_build() -> bool:
 
 
 def build(force: bool = False) -> str:
+    """OPSS_SANITIZE=1 builds with -fsanitize=address,undefined (run the pins with LD_PRELOAD=$(g++ -print-file-name=libasan.so))."""
+    global LIB
+    san = os.environ.get("OPSS_SANITIZE", "") not in ("", "0")
+    if san:
+        LIB = os.path.join(HERE, "libopss_san.so")
     if force or needs_build():
         tmp = LIB + ".tmp.%d" % os.getpid()
         cmd = ["g++", "-std=c++17", "-O2", "-fopenmp", "-fPIC", "-shared", "-ffp-contract=off",
-               "-Wall", "-Wextra", "-o", tmp, SRC]
+               "-Wall", "-Wextra"] + (["-fsanitize=address,undefined", "-fno-omit-frame-pointer", "-g"] if san else []) + ["-o", tmp, SRC]
         subprocess.run(cmd, check=True, cwd=HERE)
         os.replace(tmp, LIB)
     return LIB

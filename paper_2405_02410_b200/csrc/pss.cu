@@ -23,11 +23,13 @@
 namespace {
 
 struct DefH { pss_op op; int src; };
+struct ATermH { pss_op outer; std::vector<int> factors; };
 struct FieldH {
   std::string name;
   bool dynamic;
   std::vector<DefH> defs;
-  std::vector<pss_op> lhs;
+  std::vector<pss_op> lhs;    /* dynamic: implicit terms; intermediate: its own lhs */
+  std::vector<ATermH> aterms; /* intermediate: rhs terms that are products          */
   bool noisy;
   double D;
   int qpow;
@@ -63,8 +65,14 @@ struct pss_system {
   uint64_t step;
   std::vector<FieldH> fields;
   std::vector<TermH> terms;
-  std::vector<int> dyn_slot;
-  Program P;
+  std::vector<int> dyn_slot; /* field -> spectral source slot (dynamic fields, then product-defined intermediate fields), else -1 */
+  Program P;                 /* the launch program of the last round: groups of the dynamic equations, Eq. 18, factors of the first round */
+  /* systems with product-defined intermediate fields run one extra round of the two step kernels per dependency level:
+   * PR[k] = (factors, groups, terms) of round k for k_rows; PU[k] = (groups, slot kinds of round k, factors of the next
+   * round) for k_update.  Round nround - 1 is the dynamic equations'.  Without such fields nround = 1 and PR[0] = PU[0] = P. */
+  int nround;
+  std::vector<Program> PR, PU;
+  int nfac_max, ngrp_max; /* over the rounds: array counts and tile sizes are planned for the largest round */
   Plan plan;
   size_t csize, rsize;
   int64_t M, N; /* modes (half-spectrum), sites */
@@ -148,6 +156,7 @@ DOp link_op(const pss_system *s, const pss_op &op, int src_slot) {
   d.src = (int8_t)src_slot;
   return d;
 }
+bool real_op(const DOp &d) { return ((d.a[0] + d.a[1] + d.a[2]) & 1) == 0; }
 bool compose(const DOp &outer, const DOp &inner, DOp &r) {
   r = inner;
   r.coef = outer.coef * inner.coef;
@@ -161,11 +170,13 @@ bool compose(const DOp &outer, const DOp &inner, DOp &r) {
     r.a[j] = (int8_t)a;
   }
   r.zflags = outer.zflags | inner.zflags;
+  if (outer.den && inner.den) return false; /* one denominator per monomial */
+  r.den = outer.den ? outer.den : inner.den;
   return true;
 }
 bool same_monomial(const DOp &a, const DOp &b) {
   return a.m == b.m && a.p == b.p && a.a[0] == b.a[0] && a.a[1] == b.a[1] && a.a[2] == b.a[2] &&
-         a.zflags == b.zflags && a.src == b.src;
+         a.zflags == b.zflags && a.src == b.src && a.den == b.den;
 }
 void push_merged(std::vector<DOp> &v, const DOp &d) {
   for (DOp &e : v)
@@ -173,19 +184,22 @@ void push_merged(std::vector<DOp> &v, const DOp &d) {
   v.push_back(d);
 }
 
-/* field -> sum of monomials acting on dynamic fields (aux fields are linear in them) */
-bool flatten(const pss_system *s, std::vector<std::vector<DOp>> &flat) {
+/* field -> sum of monomials acting on spectral sources.  Dynamic fields and product-defined intermediate fields ARE
+ * sources; the other intermediate fields are linear in earlier fields and flatten onto them, each link
+ * carrying its Nyquist / q = 0 zero rules (A9, A10) and the denominator of a field with its own lhs. */
+bool flatten(const pss_system *s, const std::vector<int> &den_of, std::vector<std::vector<DOp>> &flat) {
   const int nf = (int)s->fields.size();
   flat.assign(nf, std::vector<DOp>());
   for (int f = 0; f < nf; ++f) {
     const FieldH &F = s->fields[f];
-    if (F.dynamic) {
+    if (s->dyn_slot[f] >= 0) {
       pss_op one = {1.0, 0, 0, {0, 0, 0}};
       flat[f].push_back(link_op(s, one, s->dyn_slot[f]));
       continue;
     }
     for (const DefH &d : F.defs) {
-      const DOp l = link_op(s, d.op, 0);
+      DOp l = link_op(s, d.op, 0);
+      l.den = (int8_t)den_of[f];
       for (const DOp &e : flat[d.src]) {
         DOp r;
         if (!compose(l, e, r)) return false;
@@ -196,71 +210,49 @@ bool flatten(const pss_system *s, std::vector<std::vector<DOp>> &flat) {
   return true;
 }
 
-int build_program(pss_system *s) {
-  Program &P = s->P;
-  std::memset(&P, 0, sizeof(P));
-  P.ndim = s->ndim;
-  double dV = 1.0;
-  for (int j = 0; j < 3; ++j) {
-    P.n[j] = (int32_t)s->n[j];
-    P.qs[j] = (j < s->ndim) ? 2.0 * 3.14159265358979323846 / ((double)s->n[j] * s->dx[j]) : 0.0;
-    if (j < s->ndim) dV *= s->dx[j];
-  }
-  P.nxh = (int32_t)(s->n[0] / 2 + 1);
-  P.dealias = s->dealias;
-  P.dt = s->dt;
-  P.invN = 1.0 / (double)s->N;
-  P.seed_lo = (uint32_t)(s->seed & 0xffffffffu);
-  P.seed_hi = (uint32_t)(s->seed >> 32);
+/* (factors, groups, terms) of one round: the product terms `terms` (field = target source slot) */
+struct RoundH {
+  std::vector<DFactor> fac;
+  std::vector<DGroup> grp;
+  std::vector<DTerm> term;
+};
+struct PTermH { int target; pss_op outer; std::vector<int> factors; };
 
+int build_round(const pss_system *s, const std::vector<PTermH> &terms, const std::vector<std::vector<DOp>> &flat,
+                const std::vector<int> &order_of, std::vector<DOp> &lin, RoundH &R) {
   const int nf = (int)s->fields.size();
-  s->dyn_slot.assign(nf, -1);
-  int ndyn = 0;
-  for (int f = 0; f < nf; ++f)
-    if (s->fields[f].dynamic) {
-      if (ndyn >= PSS_P_MAX_DYN) return PSS_EUNSUPPORTED;
-      s->dyn_slot[f] = ndyn++;
-    }
-  P.ndyn = ndyn;
-  std::vector<std::vector<DOp>> flat;
-  if (!flatten(s, flat)) return PSS_EUNSUPPORTED;
-
-  std::vector<DOp> lin;
-  /* factor fields: appear in a product of order >= 2 */
   std::vector<int> fac_slot(nf, -1);
-  int nfac = 0;
   for (int f = 0; f < nf; ++f) {
-    int order = 0;
-    for (const TermH &t : s->terms) {
-      if (t.factors.size() < 2) continue;
-      for (int g : t.factors)
-        if (g == f && (int)t.factors.size() > order) order = (int)t.factors.size();
-    }
-    if (order < 2) continue;
-    if (nfac >= PSS_P_MAX_FAC) return PSS_EUNSUPPORTED;
-    DFactor &F = P.fac[nfac];
+    bool used = false;
+    for (const PTermH &t : terms)
+      for (int g : t.factors) if (g == f) used = true;
+    if (!used) continue;
+    if ((int)R.fac.size() >= PSS_P_MAX_FAC) return PSS_EUNSUPPORTED;
+    DFactor F;
+    std::memset(&F, 0, sizeof(F));
     F.lin_beg = (int16_t)lin.size();
     for (const DOp &e : flat[f]) lin.push_back(e);
     F.lin_end = (int16_t)lin.size();
-    F.order = (int16_t)order;
-    fac_slot[f] = nfac++;
+    F.order = (int16_t)order_of[f];
+    fac_slot[f] = (int)R.fac.size();
+    R.fac.push_back(F);
   }
-  P.nfac = nfac;
   /* groups of product terms: same target, same outer monomial (coef moves into the term) */
-  int ngrp = 0, nterm = 0;
   std::vector<std::vector<DTerm>> gterms;
-  for (const TermH &t : s->terms) {
-    if (t.factors.size() < 2) continue;
-    DOp o = link_op(s, t.outer, s->dyn_slot[t.field]);
+  for (const PTermH &t : terms) {
+    DOp o = link_op(s, t.outer, t.target);
     o.coef = 1.0;
     int g = -1;
-    for (int i = 0; i < ngrp; ++i)
-      if (P.grp[i].target == s->dyn_slot[t.field] && same_monomial(P.grp[i].outer, o)) g = i;
+    for (size_t i = 0; i < R.grp.size(); ++i)
+      if (R.grp[i].target == t.target && same_monomial(R.grp[i].outer, o)) g = (int)i;
     if (g < 0) {
-      if (ngrp >= PSS_P_MAX_GRP) return PSS_EUNSUPPORTED;
-      g = ngrp++;
-      P.grp[g].outer = o;
-      P.grp[g].target = (int16_t)s->dyn_slot[t.field];
+      if ((int)R.grp.size() >= PSS_P_MAX_GRP) return PSS_EUNSUPPORTED;
+      DGroup G;
+      std::memset(&G, 0, sizeof(G));
+      G.outer = o;
+      G.target = (int16_t)t.target;
+      g = (int)R.grp.size();
+      R.grp.push_back(G);
       gterms.push_back(std::vector<DTerm>());
     }
     DTerm dt;
@@ -268,26 +260,132 @@ int build_program(pss_system *s) {
     dt.coef = t.outer.coef;
     dt.nf = (int8_t)t.factors.size();
     for (size_t i = 0; i < t.factors.size(); ++i) dt.f[i] = (int8_t)fac_slot[t.factors[i]];
-    gterms[g].push_back(dt);
-    ++nterm;
+    gterms[(size_t)g].push_back(dt);
   }
-  if (nterm > PSS_P_MAX_TERM) return PSS_EUNSUPPORTED;
-  int tpos = 0;
-  for (int g = 0; g < ngrp; ++g) {
-    P.grp[g].term_beg = (int16_t)tpos;
-    for (const DTerm &dt : gterms[g]) P.term[tpos++] = dt;
-    P.grp[g].term_end = (int16_t)tpos;
+  for (size_t g = 0; g < R.grp.size(); ++g) {
+    R.grp[g].term_beg = (int16_t)R.term.size();
+    for (const DTerm &dt : gterms[g]) R.term.push_back(dt);
+    R.grp[g].term_end = (int16_t)R.term.size();
   }
-  P.ngrp = ngrp;
-  P.nterm = nterm;
-  /* per dynamic field: lhs, explicit linear terms, noise */
+  if ((int)R.term.size() > PSS_P_MAX_TERM) return PSS_EUNSUPPORTED;
+  return PSS_OK;
+}
+
+void put_round(Program &P, const RoundH &facs, const RoundH &grps) {
+  P.nfac = (int32_t)facs.fac.size();
+  for (size_t i = 0; i < facs.fac.size(); ++i) P.fac[i] = facs.fac[i];
+  P.ngrp = (int32_t)grps.grp.size();
+  for (size_t i = 0; i < grps.grp.size(); ++i) P.grp[i] = grps.grp[i];
+  P.nterm = (int32_t)grps.term.size();
+  for (size_t i = 0; i < grps.term.size(); ++i) P.term[i] = grps.term[i];
+}
+
+int build_program(pss_system *s) {
+  Program base;
+  std::memset(&base, 0, sizeof(base));
+  base.ndim = s->ndim;
+  double dV = 1.0;
+  for (int j = 0; j < 3; ++j) {
+    base.n[j] = (int32_t)s->n[j];
+    base.qs[j] = (j < s->ndim) ? 2.0 * 3.14159265358979323846 / ((double)s->n[j] * s->dx[j]) : 0.0;
+    if (j < s->ndim) dV *= s->dx[j];
+  }
+  base.nxh = (int32_t)(s->n[0] / 2 + 1);
+  base.dealias = s->dealias;
+  base.dt = s->dt;
+  base.invN = 1.0 / (double)s->N;
+  base.seed_lo = (uint32_t)(s->seed & 0xffffffffu);
+  base.seed_hi = (uint32_t)(s->seed >> 32);
+
+  const int nf = (int)s->fields.size();
+  /* spectral sources: dynamic fields first, then the intermediate fields that are defined by products */
+  s->dyn_slot.assign(nf, -1);
+  int nsrc = 0, ndyn = 0;
+  for (int f = 0; f < nf; ++f)
+    if (s->fields[f].dynamic) { s->dyn_slot[f] = nsrc++; ++ndyn; }
+  for (int f = 0; f < nf; ++f)
+    if (!s->fields[f].dynamic && !s->fields[f].aterms.empty()) s->dyn_slot[f] = nsrc++;
+  if (nsrc > PSS_P_MAX_DYN) return PSS_EUNSUPPORTED;
+  base.ndyn = nsrc;
+  const bool multi = nsrc > ndyn;
+  if (multi && (s->ndim == 1 || s->nrep != 1)) return PSS_EUNSUPPORTED; /* rounds: 2D/3D single systems */
+
+  std::vector<DOp> lin;
+  /* denominators of the intermediate fields with their own lhs: real-valued monomials only */
+  std::vector<int> den_of(nf, 0);
   for (int f = 0; f < nf; ++f) {
-    if (!s->fields[f].dynamic) continue;
     const FieldH &F = s->fields[f];
-    DDyn &d = P.dyn[s->dyn_slot[f]];
+    if (F.dynamic || F.lhs.empty()) continue;
+    if (base.nden >= PSS_P_MAX_DEN) return PSS_EUNSUPPORTED;
+    DDen &D = base.den[base.nden];
+    D.beg = (int16_t)lin.size();
+    std::vector<DOp> tmp;
+    for (const pss_op &op : F.lhs) {
+      DOp d = link_op(s, op, 0);
+      if (!real_op(d)) return PSS_EUNSUPPORTED;
+      push_merged(tmp, d);
+    }
+    for (const DOp &e : tmp) lin.push_back(e);
+    D.end = (int16_t)lin.size();
+    den_of[f] = ++base.nden;
+  }
+  std::vector<std::vector<DOp>> flat;
+  if (!flatten(s, den_of, flat)) return PSS_EUNSUPPORTED;
+
+  /* highest product order every field appears in, over ALL products */
+  std::vector<int> order_of(nf, 0);
+  auto see = [&](const std::vector<int> &factors) {
+    if (factors.size() < 2) return;
+    for (int g : factors) if ((int)factors.size() > order_of[g]) order_of[g] = (int)factors.size();
+  };
+  for (const TermH &t : s->terms) see(t.factors);
+  for (const FieldH &F : s->fields) for (const ATermH &t : F.aterms) see(t.factors);
+
+  /* dependency level of every field: sources of level l are assigned in round l (dynamic fields: level 0, stepped last) */
+  std::vector<int> level(nf, 0);
+  int lmax = 0;
+  for (int f = 0; f < nf; ++f) {
+    const FieldH &F = s->fields[f];
+    if (F.dynamic) continue;
+    int lv = 0;
+    for (const DefH &d : F.defs) lv = std::max(lv, level[d.src]);
+    if (!F.aterms.empty()) {
+      for (const ATermH &t : F.aterms) for (int g : t.factors) lv = std::max(lv, level[g]);
+      lv += 1;
+    }
+    level[f] = lv;
+    lmax = std::max(lmax, lv);
+  }
+  s->nround = lmax + 1;
+
+  /* rounds 0 .. lmax-1: the product-defined intermediate fields of level round + 1; round lmax: the dynamic equations */
+  std::vector<RoundH> R((size_t)s->nround);
+  for (int k = 0; k < s->nround; ++k) {
+    std::vector<PTermH> pt;
+    if (k < lmax) {
+      for (int f = 0; f < nf; ++f)
+        if (s->dyn_slot[f] >= 0 && !s->fields[f].dynamic && level[f] == k + 1)
+          for (const ATermH &t : s->fields[f].aterms) { PTermH x; x.target = s->dyn_slot[f]; x.outer = t.outer; x.factors = t.factors; pt.push_back(x); }
+    } else {
+      for (const TermH &t : s->terms)
+        if (t.factors.size() >= 2) { PTermH x; x.target = s->dyn_slot[t.field]; x.outer = t.outer; x.factors = t.factors; pt.push_back(x); }
+    }
+    const int rc = build_round(s, pt, flat, order_of, lin, R[(size_t)k]);
+    if (rc != PSS_OK) return rc;
+  }
+
+  /* per source slot: lhs, explicit linear terms, noise (dynamic) / linear part of the definition, denominator (intermediate) */
+  std::vector<DDyn> slots((size_t)nsrc);
+  std::vector<int> slot_level((size_t)nsrc, 0);
+  for (int f = 0; f < nf; ++f) {
+    if (s->dyn_slot[f] < 0) continue;
+    const FieldH &F = s->fields[f];
+    DDyn &d = slots[(size_t)s->dyn_slot[f]];
+    std::memset(&d, 0, sizeof(d));
     d.field_id = f;
+    slot_level[(size_t)s->dyn_slot[f]] = level[f];
     d.lhs_beg = (int16_t)lin.size();
-    {
+    if (F.dynamic) {
       std::vector<DOp> tmp;
       for (const pss_op &op : F.lhs) push_merged(tmp, link_op(s, op, s->dyn_slot[f]));
       for (const DOp &e : tmp) lin.push_back(e);
@@ -296,33 +394,63 @@ int build_program(pss_system *s) {
     d.lin_beg = (int16_t)lin.size();
     {
       std::vector<DOp> tmp;
-      for (const TermH &t : s->terms) {
-        if (t.field != f || t.factors.size() != 1) continue;
-        const DOp l = link_op(s, t.outer, 0);
-        for (const DOp &e : flat[t.factors[0]]) {
-          DOp r;
-          if (!compose(l, e, r)) return PSS_EUNSUPPORTED;
-          push_merged(tmp, r);
+      if (F.dynamic) {
+        for (const TermH &t : s->terms) {
+          if (t.field != f || t.factors.size() != 1) continue;
+          const DOp l = link_op(s, t.outer, 0);
+          for (const DOp &e : flat[t.factors[0]]) {
+            DOp r;
+            if (!compose(l, e, r)) return PSS_EUNSUPPORTED;
+            push_merged(tmp, r);
+          }
         }
+      } else {
+        for (const DefH &df : F.defs) { /* linear part of a product-defined intermediate field; its den applies to the whole sum */
+          const DOp l = link_op(s, df.op, 0);
+          for (const DOp &e : flat[df.src]) {
+            DOp r;
+            if (!compose(l, e, r)) return PSS_EUNSUPPORTED;
+            push_merged(tmp, r);
+          }
+        }
+        d.den = (int16_t)den_of[f];
       }
       for (const DOp &e : tmp) lin.push_back(e);
     }
     d.lin_end = (int16_t)lin.size();
-    d.noisy = F.noisy ? 1 : 0;
+    d.noisy = (F.dynamic && F.noisy) ? 1 : 0;
     d.noise_qpow = (int16_t)F.qpow;
     d.noise_c = 2.0 * F.D * s->dt * (double)s->N / dV;
   }
   if (lin.size() > PSS_P_MAX_LIN) return PSS_EUNSUPPORTED;
-  for (size_t i = 0; i < lin.size(); ++i) P.lin[i] = lin[i];
-  P.nlin = (int32_t)lin.size();
-  P.any_invq = 0;
-  for (const DOp &d : lin) if (d.p > 0) P.any_invq = 1;
-  for (int g = 0; g < P.ngrp; ++g) if (P.grp[g].outer.p > 0) P.any_invq = 1;
+  for (size_t i = 0; i < lin.size(); ++i) base.lin[i] = lin[i];
+  base.nlin = (int32_t)lin.size();
+  base.any_invq = 0;
+  for (const DOp &d : lin) if (d.p > 0) base.any_invq = 1;
+  for (const RoundH &r : R) for (const DGroup &g : r.grp) if (g.outer.p > 0) base.any_invq = 1;
+
+  /* launch programs */
+  s->PR.assign((size_t)s->nround, base);
+  s->PU.assign((size_t)s->nround, base);
+  for (int k = 0; k < s->nround; ++k) {
+    put_round(s->PR[(size_t)k], R[(size_t)k], R[(size_t)k]);
+    put_round(s->PU[(size_t)k], R[(size_t)((k + 1) % s->nround)], R[(size_t)k]);
+    for (int i = 0; i < nsrc; ++i) {
+      DDyn d = slots[(size_t)i];
+      const bool is_dyn = s->fields[(size_t)d.field_id].dynamic;
+      if (k == lmax) d.kind = is_dyn ? PSS_SLOT_STEP : PSS_SLOT_KEEP;
+      else d.kind = (!is_dyn && slot_level[(size_t)i] == k + 1) ? PSS_SLOT_ASSIGN : PSS_SLOT_KEEP;
+      s->PR[(size_t)k].dyn[i] = d;
+      s->PU[(size_t)k].dyn[i] = d;
+    }
+  }
+  s->P = s->PU[(size_t)lmax];
+  Program &P = s->P;
   /* radial fast path (pss_program.h): L and the outer operator polynomials in q^2, every factor a polynomial in q^2
    * times one derivative monomial */
   {
-    auto radial = [](const DOp &d) { return d.p == 0 && d.a[0] == 0 && d.a[1] == 0 && d.a[2] == 0 && d.zflags == 0 && d.m <= 4; };
-    bool ok = env_int("PSS_RADIAL", 1) != 0 && P.ndyn == 1 && P.ngrp <= 1 && P.dyn[0].lin_beg == P.dyn[0].lin_end;
+    auto radial = [](const DOp &d) { return d.p == 0 && d.a[0] == 0 && d.a[1] == 0 && d.a[2] == 0 && d.zflags == 0 && d.m <= 4 && d.den == 0; };
+    bool ok = env_int("PSS_RADIAL", 1) != 0 && !multi && P.nden == 0 && P.ndyn == 1 && P.ngrp <= 1 && P.dyn[0].lin_beg == P.dyn[0].lin_end;
     if (ok && P.dyn[0].noisy && (P.dyn[0].noise_qpow < 0 || (P.dyn[0].noise_qpow & 1) || P.dyn[0].noise_qpow > 14)) ok = false;
     for (int e = P.dyn[0].lhs_beg; ok && e < P.dyn[0].lhs_end; ++e) ok = radial(P.lin[e]);
     if (ok && P.ngrp == 1) ok = radial(P.grp[0].outer);
@@ -330,7 +458,7 @@ int build_program(pss_system *s) {
       const DOp &d0 = P.lin[P.fac[f].lin_beg];
       for (int e = P.fac[f].lin_beg; ok && e < P.fac[f].lin_end; ++e) {
         const DOp &d = P.lin[e];
-        ok = d.p == 0 && d.m <= 4 && (d.zflags & 8) == 0 && d.a[0] == d0.a[0] && d.a[1] == d0.a[1] && d.a[2] == d0.a[2] &&
+        ok = d.p == 0 && d.m <= 4 && d.den == 0 && (d.zflags & 8) == 0 && d.a[0] == d0.a[0] && d.a[1] == d0.a[1] && d.a[2] == d0.a[2] &&
              d.zflags == d0.zflags && d.a[0] <= 3 && d.a[1] <= 3 && d.a[2] <= 3;
       }
       if (P.fac[f].lin_beg == P.fac[f].lin_end) ok = false;
@@ -353,6 +481,9 @@ int build_program(pss_system *s) {
         if (P.rad_a[f][0] | P.rad_a[f][1] | P.rad_a[f][2]) P.rad_ok = 2;
     }
   }
+  if (!multi) { s->PR[0] = P; s->PU[0] = P; }
+  s->nfac_max = s->ngrp_max = 0;
+  for (const Program &X : s->PR) { s->nfac_max = std::max(s->nfac_max, (int)X.nfac); s->ngrp_max = std::max(s->ngrp_max, (int)X.ngrp); }
   return PSS_OK;
 }
 
@@ -414,7 +545,6 @@ int round_threads(long long work) {
 }
 
 /* the persistent kernel of pss_fused2d.cuh: one real-coefficient field with one product group on 1024^2 fp32 */
-bool real_op(const DOp &d) { return ((d.a[0] + d.a[1] + d.a[2]) & 1) == 0; }
 bool fused2d_eligible(const pss_system *s) {
   const Program &P = s->P;
   if (env_int("PSS_FUSED", 1) == 0) return false;
@@ -430,20 +560,24 @@ bool fused2d_eligible(const pss_system *s) {
 int make_plan(pss_system *s) {
   Plan &pl = s->plan;
   std::memset(&pl, 0, sizeof(pl));
-  const Program &P = s->P;
+  Program Pm = s->P; /* counts of the largest round */
+  Pm.nfac = s->nfac_max;
+  Pm.ngrp = s->ngrp_max;
+  const Program &P = Pm;
   for (int j = 0; j < 3; ++j) pl.geo[j] = make_geo(s->n[j]);
   const size_t cs = s->csize;
   const int nxh = P.nxh;
   pl.kx_keep_max = 0;
-  for (int f = 0; f < P.nfac; ++f) {
-    int cut = nxh;
-    if (P.dealias != PSS_DEALIAS_OFF) {
-      const int nn = (P.dealias == PSS_DEALIAS_TWO_THIRDS ? 2 : P.fac[f].order) + 1;
-      cut = (int)((s->n[0] + nn - 1) / nn);
-      if (cut > nxh) cut = nxh;
+  for (const Program &X : s->PR)
+    for (int f = 0; f < X.nfac; ++f) {
+      int cut = nxh;
+      if (P.dealias != PSS_DEALIAS_OFF) {
+        const int nn = (P.dealias == PSS_DEALIAS_TWO_THIRDS ? 2 : X.fac[f].order) + 1;
+        cut = (int)((s->n[0] + nn - 1) / nn);
+        if (cut > nxh) cut = nxh;
+      }
+      if (cut > pl.kx_keep_max) pl.kx_keep_max = cut;
     }
-    if (cut > pl.kx_keep_max) pl.kx_keep_max = cut;
-  }
   pl.pdl = env_int("PSS_PDL", 1);
   pl.fused = fused2d_eligible(s) ? 1 : 0;
   if (pl.fused) {
@@ -547,8 +681,8 @@ void carve_workspace(pss_system *s) {
   const size_t arr = align_up((size_t)s->M * s->csize, 256);
   const size_t R = (size_t)s->nrep; /* arrays of one kind: [replica][field][M] */
   s->off_state = off; off += arr * (size_t)P.ndyn * R;
-  s->off_psix = off;  off += arr * (size_t)(P.nfac > 0 ? P.nfac : 0) * R;
-  s->off_phat = off;  off += arr * (size_t)(P.ngrp > 0 ? P.ngrp : 0) * R;
+  s->off_psix = off;  off += arr * (size_t)s->nfac_max * R;
+  s->off_phat = off;  off += arr * (size_t)s->ngrp_max * R;
   s->off_scratch = off; off += arr;
   s->off_ureal = off; off += align_up((size_t)s->N * s->rsize, 256);
   for (int j = 0; j < 3; ++j) { s->off_tw[j] = off; off += align_up((size_t)tw_entries(s->plan.geo[j]) * s->csize, 256); }
@@ -679,12 +813,12 @@ cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, unsigned threads, si
   return cudaLaunchKernelEx(&cfg, kernel, args...);
 }
 
-template <typename T> int launch_mid(pss_system *s, int sgn, size_t off, int nbatch, int kx_count, bool factor_mask = false, int nrep = 1) {
+template <typename T> int launch_mid(pss_system *s, int sgn, size_t off, int nbatch, int kx_count, const Program *Pf = nullptr, int nrep = 1) {
   MidArgs<T> a;
   std::memset(&a, 0, sizeof(a));
   a.nx = (int)s->n[0];
-  if (factor_mask && s->P.dealias != PSS_DEALIAS_OFF)
-    for (int f = 0; f < nbatch; ++f) a.nn[f] = (s->P.dealias == PSS_DEALIAS_TWO_THIRDS ? 2 : s->P.fac[f].order) + 1;
+  if (Pf && Pf->dealias != PSS_DEALIAS_OFF) /* Pf: the program whose factor list is being transformed (mask per factor) */
+    for (int f = 0; f < nbatch; ++f) a.nn[f] = (Pf->dealias == PSS_DEALIAS_TWO_THIRDS ? 2 : Pf->fac[f].order) + 1;
   a.arr = carr<T>(s, off, 0);
   a.tw = twp<T>(s, 1);
   a.M = arr_stride(s);
@@ -703,8 +837,7 @@ template <typename T> int launch_mid(pss_system *s, int sgn, size_t off, int nba
   return PSS_OK;
 }
 
-template <typename T> int launch_update(pss_system *s, int prologue, uint64_t step) {
-  const Program &P = s->P;
+template <typename T> int launch_update(pss_system *s, int prologue, uint64_t step, const Program &P) {
   UpdArgs<T> a;
   a.state = carr<T>(s, s->off_state, 0);
   a.psix = carr<T>(s, s->off_psix, 0);
@@ -728,12 +861,11 @@ template <typename T> int launch_update(pss_system *s, int prologue, uint64_t st
   else launch_pdl(k_update<T, 0>, grid, s->plan.upd_threads, s->plan.upd_smem, s->stream, pdl, P, a);
   prof_mark(s, KIND_UPDATE, false);
   CKL("k_update");
-  if (s->ndim == 3 && P.nfac > 0) return launch_mid<T>(s, +1, s->off_psix, P.nfac, s->plan.kx_keep_max, true, s->nrep);
+  if (s->ndim == 3 && P.nfac > 0) return launch_mid<T>(s, +1, s->off_psix, P.nfac, s->plan.kx_keep_max, &P, s->nrep);
   return PSS_OK;
 }
 
-template <typename T> int launch_rows(pss_system *s) {
-  const Program &P = s->P;
+template <typename T> int launch_rows(pss_system *s, const Program &P) {
   RowArgs<T> a;
   a.psix = carr<T>(s, s->off_psix, 0);
   a.phat = carr<T>(s, s->off_phat, 0);
@@ -750,7 +882,7 @@ template <typename T> int launch_rows(pss_system *s) {
   else launch_pdl(k_rows<T, false>, grid, s->plan.row_threads, s->plan.row_smem, s->stream, pdl, P, a);
   prof_mark(s, KIND_ROWS, false);
   CKL("k_rows");
-  if (s->ndim == 3) return launch_mid<T>(s, -1, s->off_phat, P.ngrp, P.nxh, false, s->nrep);
+  if (s->ndim == 3) return launch_mid<T>(s, -1, s->off_phat, P.ngrp, P.nxh, nullptr, s->nrep);
   return PSS_OK;
 }
 
@@ -854,13 +986,18 @@ template <typename T> int do_steps(pss_system *s, int64_t nsteps) {
   }
   int rc;
   if (s->plan.fused) return launch_fused(s, nsteps);
-  if (P.nfac > 0 && !s->psix_valid) {
-    if ((rc = launch_update<T>(s, 1, s->step)) != PSS_OK) return rc;
+  /* one round of (k_rows, k_update) per dependency level of the product-defined intermediate fields,
+   * the dynamic equations last; without such fields this is the single pair of round 0 */
+  const int last = s->nround - 1;
+  if (s->nfac_max > 0 && !s->psix_valid) {
+    if ((rc = launch_update<T>(s, 1, s->step, s->PU[(size_t)last])) != PSS_OK) return rc;
     s->psix_valid = true;
   }
   for (int64_t i = 0; i < nsteps; ++i) {
-    if (P.ngrp > 0 && (rc = launch_rows<T>(s)) != PSS_OK) return rc;
-    if ((rc = launch_update<T>(s, 0, s->step)) != PSS_OK) return rc;
+    for (int k = 0; k <= last; ++k) {
+      if (s->PR[(size_t)k].ngrp > 0 && (rc = launch_rows<T>(s, s->PR[(size_t)k])) != PSS_OK) return rc;
+      if ((rc = launch_update<T>(s, 0, s->step, s->PU[(size_t)k])) != PSS_OK) return rc;
+    }
     s->step += 1;
   }
   return PSS_OK;
@@ -1063,6 +1200,33 @@ int pss_add_aux_def(pss_system *s, int aux, const pss_op *op, int src) {
   return PSS_OK;
 }
 
+int pss_add_aux_lhs(pss_system *s, int aux, const pss_op *op) {
+  if (!s) return PSS_EINVAL;
+  if (s->finalized) return PSS_ESTATE;
+  if (!fid_ok(s, aux) || !op_ok(s, op)) return PSS_EINVAL;
+  if (s->fields[aux].dynamic) return PSS_EINVAL;
+  s->fields[aux].lhs.push_back(*op);
+  return PSS_OK;
+}
+
+int pss_add_aux_term(pss_system *s, int aux, const pss_op *outer, int nfactors, const int *factor_fields) {
+  if (!s) return PSS_EINVAL;
+  if (s->finalized) return PSS_ESTATE;
+  if (!fid_ok(s, aux) || !op_ok(s, outer) || !factor_fields) return PSS_EINVAL;
+  if (s->fields[aux].dynamic) return PSS_EINVAL;
+  if (nfactors < 2) return PSS_EINVAL; /* one factor is pss_add_aux_def */
+  if (nfactors > 4) return PSS_EUNSUPPORTED;
+  ATermH t; t.outer = *outer;
+  for (int i = 0; i < nfactors; ++i) {
+    const int g = factor_fields[i];
+    if (!fid_ok(s, g)) return PSS_EINVAL;
+    if (!s->fields[g].dynamic && g >= aux) return PSS_EINVAL; /* dynamic or EARLIER intermediate fields only (A12) */
+    t.factors.push_back(g);
+  }
+  s->fields[aux].aterms.push_back(t);
+  return PSS_OK;
+}
+
 int pss_add_term(pss_system *s, int field, const pss_op *outer, int nfactors, const int *factor_fields) {
   if (!s) return PSS_EINVAL;
   if (s->finalized) return PSS_ESTATE;
@@ -1123,7 +1287,7 @@ int pss_finalize(pss_system *s, size_t *workspace_bytes) {
   for (const FieldH &f : s->fields) ndyn += f.dynamic ? 1 : 0;
   if (ndyn == 0) return PSS_EINVAL;
   for (const FieldH &f : s->fields)
-    if (!f.dynamic && f.defs.empty()) return PSS_EINVAL;
+    if (!f.dynamic && f.defs.empty() && f.aterms.empty()) return PSS_EINVAL;
   if (s->fields.size() > 0xffff) return PSS_EUNSUPPORTED;
   int rc = build_program(s);
   if (rc != PSS_OK) return rc;
@@ -1245,8 +1409,9 @@ int pss_profile_step(pss_system *s, int64_t nsteps, double ms_per_launch[4], int
     rc = launch_fused(s, 0);
     if (rc != PSS_OK) return rc;
   }
-  if (!s->plan.fused && s->P.nfac > 0 && !s->psix_valid) {
-    rc = (s->prec == PSS_F32) ? launch_update<float>(s, 1, s->step) : launch_update<double>(s, 1, s->step);
+  if (!s->plan.fused && s->nfac_max > 0 && !s->psix_valid) {
+    rc = (s->prec == PSS_F32) ? launch_update<float>(s, 1, s->step, s->PU[(size_t)(s->nround - 1)])
+                              : launch_update<double>(s, 1, s->step, s->PU[(size_t)(s->nround - 1)]);
     if (rc != PSS_OK) return rc;
     s->psix_valid = true;
   }

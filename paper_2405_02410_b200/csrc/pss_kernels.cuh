@@ -72,6 +72,7 @@ template <typename T> __device__ __forceinline__ ModeQ<T> line_mode(const Progra
   else { mq.q[1] = ql; mq.q[2] = (T)0; mq.nyq = l.nyq | (last_nyq << 1); }
   mq.q2 = l.q2line + ql * ql;
   mq.rq = (P.any_invq && mq.q2 > (T)0) ? (T)1 / sqrt(mq.q2) : (T)0;
+  if (P.nden > 0) fill_rden<T>(P, mq);
   return mq;
 }
 template <typename T> __device__ __forceinline__ T horner4(const T (&c)[5], T x) {
@@ -159,7 +160,19 @@ __global__ void __launch_bounds__(256, sizeof(T) == 4 ? PSS_MINB : 2) k_update(c
         C out[PSS_P_MAX_DYN];
 #pragma unroll
         for (int i = 0; i < PSS_P_MAX_DYN; ++i) {
-          if (i < P.ndyn) {
+          if (i < P.ndyn && P.dyn[i].kind != PSS_SLOT_STEP) {
+            /* an intermediate field defined by products: (re)assigned in its own round, else kept */
+            const DDyn &d = P.dyn[i];
+            out[i] = phi[i];
+            if (d.kind == PSS_SLOT_ASSIGN) {
+              C N = zero;
+              for (int g = 0; g < P.ngrp; ++g)
+                if (P.grp[g].target == i) N = cadd(N, cmul(eval_op<T>(P.grp[g].outer, mq), srow[g * W]));
+              for (int e = d.lin_beg; e < d.lin_end; ++e) N = cadd(N, cmul(eval_op<T>(P.lin[e], mq), sel4(phi, P.lin[e].src)));
+              const T rd = d.den ? mq.rden[d.den - 1] : (T)1;
+              out[i] = mk<C, T>(N.x * rd, N.y * rd);
+            }
+          } else if (i < P.ndyn) {
             const DDyn &d = P.dyn[i];
             C N = zero;
             for (int g = 0; g < P.ngrp; ++g)
@@ -185,7 +198,7 @@ __global__ void __launch_bounds__(256, sizeof(T) == 4 ? PSS_MINB : 2) k_update(c
 #pragma unroll
         for (int i = 0; i < PSS_P_MAX_DYN; ++i)
           if (i < P.ndyn) {
-            st_base[(size_t)i * A.M + gi] = out[i];
+            if (P.dyn[i].kind != PSS_SLOT_KEEP) st_base[(size_t)i * A.M + gi] = out[i];
             srow[i * W] = out[i];
           }
       } else {

@@ -13,10 +13,13 @@ template <typename T> struct ModeQ {
   T q[3];
   T q2;
   T rq;    /* 1/|q| (0 at q = 0, A10); filled only when the program has a 1/q keyword (Program::any_invq) */
+  T rden[PSS_P_MAX_DEN]; /* 1/den_i(q) of the intermediate fields with an lhs (0 where den vanishes); filled when Program::nden > 0 */
   int nyq; /* bit j set: k_j is the Nyquist index of axis j */
 };
 
 __device__ __forceinline__ int signed_index(int k, int n) { return (k <= (n >> 1)) ? k : k - n; }
+
+template <typename T> __device__ __forceinline__ void fill_rden(const Program &P, ModeQ<T> &mq);
 
 template <typename T> __device__ __forceinline__ ModeQ<T> make_mode(const Program &P, int k0, int k1, int k2) {
   ModeQ<T> mq;
@@ -34,6 +37,7 @@ template <typename T> __device__ __forceinline__ ModeQ<T> make_mode(const Progra
     mq.q2 += mq.q[j] * mq.q[j];
   }
   mq.rq = (P.any_invq && mq.q2 > (T)0) ? (T)1 / sqrt(mq.q2) : (T)0;
+  if (P.nden > 0) fill_rden<T>(P, mq);
   return mq;
 }
 
@@ -42,6 +46,7 @@ template <typename T> __device__ __forceinline__ typename cplx_of<T>::type eval_
   typedef typename cplx_of<T>::type C;
   if ((op.zflags & 7 & mq.nyq) || ((op.zflags & 8) && mq.q2 == (T)0)) return mk<C, T>((T)0, (T)0);
   T r = (T)op.coef;
+  if (op.den) r *= mq.rden[op.den - 1];
   {
     T bq = mq.q2;
     for (int m = op.m; m > 0; m >>= 1) { if (m & 1) r *= bq; bq *= bq; }
@@ -62,6 +67,19 @@ template <typename T> __device__ __forceinline__ typename cplx_of<T>::type eval_
     case 1: return mk<C, T>((T)0, r);
     case 2: return mk<C, T>(-r, (T)0);
     default: return mk<C, T>((T)0, -r);
+  }
+}
+
+/* 1/den(q) of every lhs polynomial; called by the mode constructors when the program has any */
+template <typename T> __device__ __forceinline__ void fill_rden(const Program &P, ModeQ<T> &mq) {
+#pragma unroll
+  for (int i = 0; i < PSS_P_MAX_DEN; ++i) {
+    mq.rden[i] = (T)0;
+    if (i < P.nden) {
+      T d = (T)0;
+      for (int e = P.den[i].beg; e < P.den[i].end; ++e) d += eval_op<T>(P.lin[e], mq).x;
+      mq.rden[i] = (d == (T)0) ? (T)0 : (T)1 / d;
+    }
   }
 }
 
@@ -259,11 +277,12 @@ template <typename T> __device__ __forceinline__ T noise_amp(const DDyn &d, cons
   return sqrt((T)d.noise_c * qa);
 }
 
+/* v[i] for a run-time i without local-memory indexing (v lives in registers) */
 template <typename C> __device__ __forceinline__ C sel4(const C *v, int i) {
   C r = v[0];
-  if (i == 1) r = v[1];
-  if (i == 2) r = v[2];
-  if (i == 3) r = v[3];
+#pragma unroll
+  for (int j = 1; j < PSS_P_MAX_DYN; ++j)
+    if (i == j) r = v[j];
   return r;
 }
 

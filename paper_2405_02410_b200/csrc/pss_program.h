@@ -12,13 +12,15 @@
 #define PSS_PROGRAM_H
 #include <stdint.h>
 
-#define PSS_P_MAX_DYN 4
+#define PSS_P_MAX_DYN 6 /* spectral sources: dynamic fields + product-defined intermediate fields */
+#define PSS_P_MAX_DEN 2
 #define PSS_P_MAX_FAC 12
 #define PSS_P_MAX_GRP 8
 #define PSS_P_MAX_TERM 32
 #define PSS_P_MAX_LIN 96
 
-/* coef (q^2)^m |q|^-p prod_j (i q_j)^a[j] acting on dynamic field `src`.
+/* coef (q^2)^m |q|^-p prod_j (i q_j)^a[j] / den(q) acting on spectral source `src`.
+ * den: 0 = none, i > 0 = denominator i - 1 of Program::den (an intermediate field with its own lhs).
  * zflags bit j (j<3): the monomial is 0 at the Nyquist index of axis j (reading A9, applied link by
  * link before flattening); bit 3: it is 0 at q = 0 (reading A10). */
 struct DOp {
@@ -27,7 +29,7 @@ struct DOp {
   int8_t a[3];
   uint8_t zflags;
   int8_t src;
-  int8_t pad_;
+  int8_t den;
 };
 
 /* one product term of a group: coef * prod_{i<nf} factor[f[i]](x) */
@@ -54,7 +56,16 @@ struct DGroup {
   int16_t pad_;
 };
 
+/* denominator polynomial of an intermediate field's lhs: den(q) = sum_{e in [beg,end)} lin[e](q), real-valued monomials;
+ * 1/den is 0 where den vanishes (reading A10) */
+struct DDen { int16_t beg, end; };
+
+/* one spectral source (a state array): a dynamic field, or an intermediate field defined by products, which is
+ * re-evaluated every step in its own round of the two step kernels */
+enum { PSS_SLOT_STEP = 0, PSS_SLOT_ASSIGN = 1, PSS_SLOT_KEEP = 2 };
 struct DDyn {
+  int16_t kind;             /* this launch: STEP = Eq. 18; ASSIGN = (sum of its groups and linear terms) / den; KEEP = untouched */
+  int16_t den;              /* ASSIGN: 0 = none, i > 0 = Program::den[i - 1]                           */
   int16_t lhs_beg, lhs_end; /* L_q = - sum lin[e](q)                  (dt phi + lhs = rhs, A3) */
   int16_t lin_beg, lin_end; /* explicit linear terms sum lin[e](q) phi_src(q)   (A8)          */
   double noise_c;           /* 2 D dt N / dV                           (A1)                   */
@@ -74,6 +85,8 @@ struct Program {
   uint32_t seed_lo, seed_hi;
   int32_t ndyn, nfac, ngrp, nterm, nlin;
   int32_t any_invq; /* some monomial uses the 1/q keyword: the kernels then evaluate 1/|q| once per mode */
+  int32_t nden;
+  DDen den[PSS_P_MAX_DEN];
   DDyn dyn[PSS_P_MAX_DYN];
   DFactor fac[PSS_P_MAX_FAC];
   DGroup grp[PSS_P_MAX_GRP];
