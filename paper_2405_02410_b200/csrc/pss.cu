@@ -702,9 +702,10 @@ template <typename T> const typename cplx_of<T>::type *twp(pss_system *s, int ax
 }
 
 template <typename T> int set_attrs(pss_system *s) {
-  CK(cudaFuncSetAttribute(k_update<T, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_MAX));
-  CK(cudaFuncSetAttribute(k_update<T, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_MAX));
-  CK(cudaFuncSetAttribute(k_update<T, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_MAX));
+  CK(cudaFuncSetAttribute(k_update<T, 0, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_MAX));
+  CK(cudaFuncSetAttribute(k_update<T, 0, PSS_P_MAX_DYN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_MAX));
+  CK(cudaFuncSetAttribute(k_update<T, 1, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_MAX));
+  CK(cudaFuncSetAttribute(k_update<T, 2, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_MAX));
   CK(cudaFuncSetAttribute(k_rows<T, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_MAX));
   CK(cudaFuncSetAttribute(k_rows<T, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_MAX));
   CK(cudaFuncSetAttribute(k_mid<-1, T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_MAX));
@@ -856,9 +857,10 @@ template <typename T> int launch_update(pss_system *s, int prologue, uint64_t st
   prof_mark(s, KIND_UPDATE, true);
   const dim3 grid((unsigned)s->plan.upd_blocks, (unsigned)s->nrep);
   const bool pdl = s->plan.pdl != 0;
-  if (P.rad_ok == 1) launch_pdl(k_update<T, 1>, grid, s->plan.upd_threads, s->plan.upd_smem, s->stream, pdl, P, a);
-  else if (P.rad_ok == 2) launch_pdl(k_update<T, 2>, grid, s->plan.upd_threads, s->plan.upd_smem, s->stream, pdl, P, a);
-  else launch_pdl(k_update<T, 0>, grid, s->plan.upd_threads, s->plan.upd_smem, s->stream, pdl, P, a);
+  if (P.rad_ok == 1) launch_pdl(k_update<T, 1, 1>, grid, s->plan.upd_threads, s->plan.upd_smem, s->stream, pdl, P, a);
+  else if (P.rad_ok == 2) launch_pdl(k_update<T, 2, 1>, grid, s->plan.upd_threads, s->plan.upd_smem, s->stream, pdl, P, a);
+  else if (P.ndyn <= 2) launch_pdl(k_update<T, 0, 2>, grid, s->plan.upd_threads, s->plan.upd_smem, s->stream, pdl, P, a);
+  else launch_pdl(k_update<T, 0, PSS_P_MAX_DYN>, grid, s->plan.upd_threads, s->plan.upd_smem, s->stream, pdl, P, a);
   prof_mark(s, KIND_UPDATE, false);
   CKL("k_update");
   if (s->ndim == 3 && P.nfac > 0) return launch_mid<T>(s, +1, s->off_psix, P.nfac, s->plan.kx_keep_max, &P, s->nrep);

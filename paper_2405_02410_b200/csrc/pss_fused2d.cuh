@@ -268,14 +268,14 @@ __global__ void __launch_bounds__(THREADS, 1) k_fused2d(const __grid_constant__ 
       if (colw) {
         const int ky = kyb + 16 * (r & 3) + 256 * (r >> 2);
         const ModeQ<float> mq = make_mode<float>(P, kx, ky, 0);
-        t.x = dt * eval_op<float>(P.grp[0].outer, mq).x;
+        t.x = dt * eval_op<float>(P, P.grp[0].outer, mq).x;
         float Lq = 0.f;
-        for (int e = D0.lhs_beg; e < D0.lhs_end; ++e) Lq -= eval_op<float>(P.lin[e], mq).x;
+        for (int e = D0.lhs_beg; e < D0.lhs_end; ++e) Lq -= eval_op<float>(P, P.lin[e], mq).x;
         t.y = 1.0f / (1.0f - dt * Lq);
         t.z = noisy ? noise_amp<float>(D0, mq) : 0.f;
         float fc = 0.f;
         if (need_inv && keep_axis(P.dealias, P.fac[0].order, ky, N)) {
-          for (int e = P.fac[0].lin_beg; e < P.fac[0].lin_end; ++e) fc += eval_op<float>(P.lin[e], mq).x;
+          for (int e = P.fac[0].lin_beg; e < P.fac[0].lin_end; ++e) fc += eval_op<float>(P, P.lin[e], mq).x;
           fc *= invN;
         }
         t.w = fc;
@@ -486,14 +486,14 @@ __global__ void __launch_bounds__(THREADS, 1) k_fused2d_pair(const __grid_consta
       const int ky = kyb + 16 * (i & 3) + 256 * (i >> 2);
       if (colw) {
         const ModeQ<float> mq = make_mode<float>(P, kx, ky, 0);
-        t.x = dt * eval_op<float>(P.grp[0].outer, mq).x;
+        t.x = dt * eval_op<float>(P, P.grp[0].outer, mq).x;
         float Lq = 0.f;
-        for (int e = D0.lhs_beg; e < D0.lhs_end; ++e) Lq -= eval_op<float>(P.lin[e], mq).x;
+        for (int e = D0.lhs_beg; e < D0.lhs_end; ++e) Lq -= eval_op<float>(P, P.lin[e], mq).x;
         t.y = 1.0f / (1.0f - dt * Lq);
         t.z = noisy ? noise_amp<float>(D0, mq) : 0.f;
         float fc = 0.f;
         if (need_inv && keep_axis(P.dealias, P.fac[0].order, ky, N)) {
-          for (int e = P.fac[0].lin_beg; e < P.fac[0].lin_end; ++e) fc += eval_op<float>(P.lin[e], mq).x;
+          for (int e = P.fac[0].lin_beg; e < P.fac[0].lin_end; ++e) fc += eval_op<float>(P, P.lin[e], mq).x;
           fc *= invN;
         }
         t.w = fc;

@@ -72,7 +72,6 @@ template <typename T> __device__ __forceinline__ ModeQ<T> line_mode(const Progra
   else { mq.q[1] = ql; mq.q[2] = (T)0; mq.nyq = l.nyq | (last_nyq << 1); }
   mq.q2 = l.q2line + ql * ql;
   mq.rq = (P.any_invq && mq.q2 > (T)0) ? (T)1 / sqrt(mq.q2) : (T)0;
-  if (P.nden > 0) fill_rden<T>(P, mq);
   return mq;
 }
 template <typename T> __device__ __forceinline__ T horner4(const T (&c)[5], T x) {
@@ -82,7 +81,8 @@ template <typename T> __device__ __forceinline__ T horner4(const T (&c)[5], T x)
 /* ------------------------------------------------------------------------------------------ */
 /* RAD: the "radial" fast path of pss_program.h: 0 = generic term interpreter, 1 = every coefficient a polynomial in
  * q^2 (Model B, diffusion), 2 = factors carry a derivative monomial on top (KPZ) */
-template <typename T, int RAD>
+/* NS: upper bound of the number of spectral sources (register arrays of the generic path); 1 for the radial paths */
+template <typename T, int RAD, int NS>
 __global__ void __launch_bounds__(256, sizeof(T) == 4 ? PSS_MINB : 2) k_update(const __grid_constant__ Program P, const UpdArgs<T> A) {
   typedef typename cplx_of<T>::type C;
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -152,14 +152,14 @@ __global__ void __launch_bounds__(256, sizeof(T) == 4 ? PSS_MINB : 2) k_update(c
           srow[0] = phi;
         }
       } else {
-      C phi[PSS_P_MAX_DYN];
+      C phi[NS];
 #pragma unroll
-      for (int i = 0; i < PSS_P_MAX_DYN; ++i) phi[i] = (i < P.ndyn) ? st_base[(size_t)i * A.M + gi] : zero;
+      for (int i = 0; i < NS; ++i) phi[i] = (i < P.ndyn) ? st_base[(size_t)i * A.M + gi] : zero;
       if (!A.prologue) {
         const ModeQ<T> mq = line_mode<T>(P, lq, k, n, qs_last);
-        C out[PSS_P_MAX_DYN];
+        C out[NS];
 #pragma unroll
-        for (int i = 0; i < PSS_P_MAX_DYN; ++i) {
+        for (int i = 0; i < NS; ++i) {
           if (i < P.ndyn && P.dyn[i].kind != PSS_SLOT_STEP) {
             /* an intermediate field defined by products: (re)assigned in its own round, else kept */
             const DDyn &d = P.dyn[i];
@@ -167,19 +167,19 @@ __global__ void __launch_bounds__(256, sizeof(T) == 4 ? PSS_MINB : 2) k_update(c
             if (d.kind == PSS_SLOT_ASSIGN) {
               C N = zero;
               for (int g = 0; g < P.ngrp; ++g)
-                if (P.grp[g].target == i) N = cadd(N, cmul(eval_op<T>(P.grp[g].outer, mq), srow[g * W]));
-              for (int e = d.lin_beg; e < d.lin_end; ++e) N = cadd(N, cmul(eval_op<T>(P.lin[e], mq), sel4(phi, P.lin[e].src)));
-              const T rd = d.den ? mq.rden[d.den - 1] : (T)1;
+                if (P.grp[g].target == i) N = cadd(N, cmul(eval_op<T>(P, P.grp[g].outer, mq), srow[g * W]));
+              for (int e = d.lin_beg; e < d.lin_end; ++e) N = cadd(N, cmul(eval_op<T>(P, P.lin[e], mq), sel_src<NS>(phi, P.lin[e].src)));
+              const T rd = d.den ? eval_rden<T>(P, d.den - 1, mq) : (T)1;
               out[i] = mk<C, T>(N.x * rd, N.y * rd);
             }
           } else if (i < P.ndyn) {
             const DDyn &d = P.dyn[i];
             C N = zero;
             for (int g = 0; g < P.ngrp; ++g)
-              if (P.grp[g].target == i) N = cadd(N, cmul(eval_op<T>(P.grp[g].outer, mq), srow[g * W]));
-            for (int e = d.lin_beg; e < d.lin_end; ++e) N = cadd(N, cmul(eval_op<T>(P.lin[e], mq), sel4(phi, P.lin[e].src)));
+              if (P.grp[g].target == i) N = cadd(N, cmul(eval_op<T>(P, P.grp[g].outer, mq), srow[g * W]));
+            for (int e = d.lin_beg; e < d.lin_end; ++e) N = cadd(N, cmul(eval_op<T>(P, P.lin[e], mq), sel_src<NS>(phi, P.lin[e].src)));
             C L = zero;
-            for (int e = d.lhs_beg; e < d.lhs_end; ++e) L = csub(L, eval_op<T>(P.lin[e], mq));
+            for (int e = d.lhs_beg; e < d.lhs_end; ++e) L = csub(L, eval_op<T>(P, P.lin[e], mq));
             C num = mk<C, T>(phi[i].x + dt * N.x, phi[i].y + dt * N.y);
             if (d.noisy) {
               const T amp = noise_amp<T>(d, mq);
@@ -196,14 +196,14 @@ __global__ void __launch_bounds__(256, sizeof(T) == 4 ? PSS_MINB : 2) k_update(c
           }
         }
 #pragma unroll
-        for (int i = 0; i < PSS_P_MAX_DYN; ++i)
+        for (int i = 0; i < NS; ++i)
           if (i < P.ndyn) {
             if (P.dyn[i].kind != PSS_SLOT_KEEP) st_base[(size_t)i * A.M + gi] = out[i];
             srow[i * W] = out[i];
           }
       } else {
 #pragma unroll
-        for (int i = 0; i < PSS_P_MAX_DYN; ++i)
+        for (int i = 0; i < NS; ++i)
           if (i < P.ndyn) srow[i * W] = phi[i];
       }
       }
@@ -262,10 +262,10 @@ __global__ void __launch_bounds__(256, sizeof(T) == 4 ? PSS_MINB : 2) k_update(c
               v = (sph == 0) ? mk<C, T>(re, im) : (sph == 1) ? mk<C, T>(-im, re) : (sph == 2) ? mk<C, T>(-re, -im) : mk<C, T>(im, -re);
             }
           } else {
-            C phi[PSS_P_MAX_DYN];
+            C phi[NS];
 #pragma unroll
-            for (int i = 0; i < PSS_P_MAX_DYN; ++i) phi[i] = (i < P.ndyn) ? srow[i * W] : zero;
-            for (int e = F.lin_beg; e < F.lin_end; ++e) v = cadd(v, cmul(eval_op<T>(P.lin[e], mq), sel4(phi, P.lin[e].src)));
+            for (int i = 0; i < NS; ++i) phi[i] = (i < P.ndyn) ? srow[i * W] : zero;
+            for (int e = F.lin_beg; e < F.lin_end; ++e) v = cadd(v, cmul(eval_op<T>(P, P.lin[e], mq), sel_src<NS>(phi, P.lin[e].src)));
             v.x *= invN;
             v.y *= invN;
           }
@@ -580,7 +580,7 @@ __global__ void __launch_bounds__(256) k_step1d(const __grid_constant__ Program 
         const DFactor &F = P.fac[f];
         if (!keep_axis(P.dealias, F.order, kx, nx)) continue;
         C v = zero;
-        for (int e = F.lin_beg; e < F.lin_end; ++e) v = cadd(v, cmul(eval_op<T>(P.lin[e], mq), sel4(phi, P.lin[e].src)));
+        for (int e = F.lin_beg; e < F.lin_end; ++e) v = cadd(v, cmul(eval_op<T>(P, P.lin[e], mq), sel_src<PSS_P_MAX_DYN>(phi, P.lin[e].src)));
         v.x *= (T)P.invN;
         v.y *= (T)P.invN;
         if (kx == 0 || 2 * kx == nx) v.y = (T)0;
@@ -621,10 +621,10 @@ __global__ void __launch_bounds__(256) k_step1d(const __grid_constant__ Program 
           const DDyn &d = P.dyn[i];
           C N = zero;
           for (int g = 0; g < P.ngrp; ++g)
-            if (P.grp[g].target == i) N = cadd(N, cmul(eval_op<T>(P.grp[g].outer, mq), srow[g]));
-          for (int e = d.lin_beg; e < d.lin_end; ++e) N = cadd(N, cmul(eval_op<T>(P.lin[e], mq), sel4(phi, P.lin[e].src)));
+            if (P.grp[g].target == i) N = cadd(N, cmul(eval_op<T>(P, P.grp[g].outer, mq), srow[g]));
+          for (int e = d.lin_beg; e < d.lin_end; ++e) N = cadd(N, cmul(eval_op<T>(P, P.lin[e], mq), sel_src<PSS_P_MAX_DYN>(phi, P.lin[e].src)));
           C L = zero;
-          for (int e = d.lhs_beg; e < d.lhs_end; ++e) L = csub(L, eval_op<T>(P.lin[e], mq));
+          for (int e = d.lhs_beg; e < d.lhs_end; ++e) L = csub(L, eval_op<T>(P, P.lin[e], mq));
           C num = mk<C, T>(phi[i].x + (T)P.dt * N.x, phi[i].y + (T)P.dt * N.y);
           if (d.noisy) {
             const T amp = noise_amp<T>(d, mq);

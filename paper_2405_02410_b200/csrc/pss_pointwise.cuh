@@ -13,13 +13,10 @@ template <typename T> struct ModeQ {
   T q[3];
   T q2;
   T rq;    /* 1/|q| (0 at q = 0, A10); filled only when the program has a 1/q keyword (Program::any_invq) */
-  T rden[PSS_P_MAX_DEN]; /* 1/den_i(q) of the intermediate fields with an lhs (0 where den vanishes); filled when Program::nden > 0 */
   int nyq; /* bit j set: k_j is the Nyquist index of axis j */
 };
 
 __device__ __forceinline__ int signed_index(int k, int n) { return (k <= (n >> 1)) ? k : k - n; }
-
-template <typename T> __device__ __forceinline__ void fill_rden(const Program &P, ModeQ<T> &mq);
 
 template <typename T> __device__ __forceinline__ ModeQ<T> make_mode(const Program &P, int k0, int k1, int k2) {
   ModeQ<T> mq;
@@ -37,16 +34,14 @@ template <typename T> __device__ __forceinline__ ModeQ<T> make_mode(const Progra
     mq.q2 += mq.q[j] * mq.q[j];
   }
   mq.rq = (P.any_invq && mq.q2 > (T)0) ? (T)1 / sqrt(mq.q2) : (T)0;
-  if (P.nden > 0) fill_rden<T>(P, mq);
   return mq;
 }
 
-/* value of one operator monomial (A9, A10) */
-template <typename T> __device__ __forceinline__ typename cplx_of<T>::type eval_op(const DOp &op, const ModeQ<T> &mq) {
+/* value of one operator monomial without its denominator (A9, A10) */
+template <typename T> __device__ __forceinline__ typename cplx_of<T>::type eval_op_nd(const DOp &op, const ModeQ<T> &mq) {
   typedef typename cplx_of<T>::type C;
   if ((op.zflags & 7 & mq.nyq) || ((op.zflags & 8) && mq.q2 == (T)0)) return mk<C, T>((T)0, (T)0);
   T r = (T)op.coef;
-  if (op.den) r *= mq.rden[op.den - 1];
   {
     T bq = mq.q2;
     for (int m = op.m; m > 0; m >>= 1) { if (m & 1) r *= bq; bq *= bq; }
@@ -70,17 +65,21 @@ template <typename T> __device__ __forceinline__ typename cplx_of<T>::type eval_
   }
 }
 
-/* 1/den(q) of every lhs polynomial; called by the mode constructors when the program has any */
-template <typename T> __device__ __forceinline__ void fill_rden(const Program &P, ModeQ<T> &mq) {
-#pragma unroll
-  for (int i = 0; i < PSS_P_MAX_DEN; ++i) {
-    mq.rden[i] = (T)0;
-    if (i < P.nden) {
-      T d = (T)0;
-      for (int e = P.den[i].beg; e < P.den[i].end; ++e) d += eval_op<T>(P.lin[e], mq).x;
-      mq.rden[i] = (d == (T)0) ? (T)0 : (T)1 / d;
-    }
+/* 1/den(q) of the lhs polynomial `id` of an intermediate field; 0 where den vanishes (A10) */
+template <typename T> __device__ __forceinline__ T eval_rden(const Program &P, int id, const ModeQ<T> &mq) {
+  T d = (T)0;
+  for (int e = P.den[id].beg; e < P.den[id].end; ++e) d += eval_op_nd<T>(P.lin[e], mq).x;
+  return (d == (T)0) ? (T)0 : (T)1 / d;
+}
+/* value of one operator monomial, denominator included (evaluated only by the monomials that carry one) */
+template <typename T> __device__ __forceinline__ typename cplx_of<T>::type eval_op(const Program &P, const DOp &op, const ModeQ<T> &mq) {
+  typename cplx_of<T>::type v = eval_op_nd<T>(op, mq);
+  if (op.den) {
+    const T r = eval_rden<T>(P, op.den - 1, mq);
+    v.x *= r;
+    v.y *= r;
   }
+  return v;
 }
 
 /* keep iff (n+1)|s(k)| < N on this axis (A4, A5, A6) */
@@ -278,10 +277,10 @@ template <typename T> __device__ __forceinline__ T noise_amp(const DDyn &d, cons
 }
 
 /* v[i] for a run-time i without local-memory indexing (v lives in registers) */
-template <typename C> __device__ __forceinline__ C sel4(const C *v, int i) {
+template <int NS, typename C> __device__ __forceinline__ C sel_src(const C *v, int i) {
   C r = v[0];
 #pragma unroll
-  for (int j = 1; j < PSS_P_MAX_DYN; ++j)
+  for (int j = 1; j < NS; ++j)
     if (i == j) r = v[j];
   return r;
 }
