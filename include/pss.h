@@ -74,6 +74,12 @@ int pss_add_linear(pss_system *, int field, const pss_op *op);
 /* intermediate field definition psi_q += coef*Op(q)*src_q; src is a dynamic
  * field or an EARLIER aux field. */
 int pss_add_aux_def(pss_system *, int aux, const pss_op *op, int src);
+/* Dirichlet frame (section V and Fig. 2: "a buffer zone of infinite stiffness in the boundaries"): at the
+ * end of every time step the field is set, in real space, to lo_value where x_axis < lo_width and to hi_value where
+ * x_axis >= n_axis - hi_width (widths in lattice sites, 0 = none; several frames of one field are applied in the order
+ * given).  This is the built-in form of the paper's callback; an arbitrary callback is a caller kernel between
+ * pss_get_field(device) and pss_set_field(device).  Dynamic fields, before pss_finalize. */
+int pss_set_frame(pss_system *, int field, int axis, int64_t lo_width, double lo_value, int64_t hi_width, double hi_value);
 /* Intermediate field with its own lhs ("psi + psi*q^2 = -q^2*phi"): den(q) psi_q = rhs_q with
  * den(q) = sum of the operators added here; psi_q = 0 where den(q) = 0 (reading A10).  None added = the bare field.
  * The CUDA path takes real-valued lhs operators (even total derivative order) and at most two such fields

@@ -182,6 +182,7 @@ static void philox4x32_10(const uint32_t c_in[4], const uint32_t k_in[2], uint32
  * ------------------------------------------------------------------------------------------ */
 struct Def { opss_op op; int src; };
 struct ATerm { opss_op outer; std::vector<int> factors; };
+struct Frame { int axis; int64_t lo_w, hi_w; double lo_v, hi_v; };
 struct Field {
   std::string name;
   bool dynamic;
@@ -190,6 +191,7 @@ struct Field {
   std::vector<ATerm> aterms;  /* aux only: rhs terms that are products of fields                  */
   std::vector<opss_op> lhs;   /* dynamic only: dt phi + sum coef Op(q) phi = rhs */
   bool noisy; double D; int qpow;
+  std::vector<Frame> frames;  /* dynamic only: Dirichlet buffer zones set at the end of every step */
   std::vector<cplx> hat;      /* half-spectrum, unnormalised forward DFT         */
 };
 struct Term { int field; opss_op outer; std::vector<int> factors; };
@@ -480,6 +482,22 @@ static void one_step(opss_system *s) {
   }
   for (int f = 0; f < nf; ++f)
     if (s->fields[f].dynamic) s->fields[f].hat.swap(N[f]);
+  /* callback at the end of the time step: the field in real space, a frame of fixed values around the
+   * boundary ("a buffer zone of infinite stiffness", Fig. 2), back to Fourier space */
+  for (int f = 0; f < nf; ++f) {
+    Field &F = s->fields[f];
+    if (!F.dynamic || F.frames.empty()) continue;
+    std::vector<double> r;
+    c2r(F.hat, r, d, nth);
+    for (const Frame &fr : F.frames) {
+      for (int64_t x = 0; x < NS; ++x) {
+        int64_t c[3] = {x % d.n[0], (x / d.n[0]) % d.n[1], x / (d.n[0] * d.n[1])};
+        if (c[fr.axis] < fr.lo_w) r[x] = fr.lo_v;
+        else if (c[fr.axis] >= d.n[fr.axis] - fr.hi_w) r[x] = fr.hi_v;
+      }
+    }
+    r2c(r, F.hat, d, nth);
+  }
   s->step += 1;
 }
 
@@ -543,6 +561,18 @@ int opss_add_aux_def(opss_system *s, int aux, const opss_op *op, int src) {
   if (!s->fields[src].dynamic && src >= aux) return OPSS_EINVAL;
   Def d; d.op = *op; d.src = src;
   s->fields[aux].defs.push_back(d);
+  return OPSS_OK;
+}
+
+int opss_set_frame(opss_system *s, int field, int axis, int64_t lo_width, double lo_value, int64_t hi_width, double hi_value) {
+  if (!s) return OPSS_EINVAL;
+  if (s->finalized) return OPSS_ESTATE;
+  if (!fid_ok(s, field) || !s->fields[field].dynamic) return OPSS_EINVAL;
+  if (axis < 0 || axis >= s->d.ndim) return OPSS_EINVAL;
+  if (lo_width < 0 || hi_width < 0 || lo_width + hi_width > s->d.n[axis]) return OPSS_EINVAL;
+  if (!std::isfinite(lo_value) || !std::isfinite(hi_value)) return OPSS_EINVAL;
+  Frame fr; fr.axis = axis; fr.lo_w = lo_width; fr.hi_w = hi_width; fr.lo_v = lo_value; fr.hi_v = hi_value;
+  s->fields[field].frames.push_back(fr);
   return OPSS_OK;
 }
 

@@ -47,6 +47,9 @@ int opss_create(opss_system **out, int ndim, const int64_t n[3], const double dx
 int opss_add_field(opss_system *, const char *name, int dynamic, int *field_id);
 int opss_add_linear(opss_system *, int field, const opss_op *op);
 int opss_add_aux_def(opss_system *, int aux, const opss_op *op, int src);
+/* Dirichlet frame (Fig. 2): at the end of every time step the field is set, in real space, to
+ * lo_value where x_axis < lo_width and to hi_value where x_axis >= n_axis - hi_width.  Dynamic fields, before finalize. */
+int opss_set_frame(opss_system *, int field, int axis, int64_t lo_width, double lo_value, int64_t hi_width, double hi_value);
 /* intermediate field with its own lhs: (sum of the ops added here)(q) * psi_q = rhs_q; psi_q = 0 where
  * the sum vanishes.  None added = the bare field. */
 int opss_add_aux_lhs(opss_system *, int aux, const opss_op *op);

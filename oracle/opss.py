@@ -48,6 +48,7 @@ def lib():
         L.opss_add_linear.argtypes = [P, C.c_int, C.POINTER(_Op)]
         L.opss_add_aux_def.argtypes = [P, C.c_int, C.POINTER(_Op), C.c_int]
         L.opss_add_term.argtypes = [P, C.c_int, C.POINTER(_Op), C.c_int, C.POINTER(C.c_int)]
+        L.opss_set_frame.argtypes = [P, C.c_int, C.c_int, C.c_int64, C.c_double, C.c_int64, C.c_double]
         L.opss_add_aux_lhs.argtypes = [P, C.c_int, C.POINTER(_Op)]
         L.opss_add_aux_term.argtypes = [P, C.c_int, C.POINTER(_Op), C.c_int, C.POINTER(C.c_int)]
         L.opss_set_noise.argtypes = [P, C.c_int, C.c_double, C.c_int]
@@ -129,6 +130,9 @@ class System:
 
     def add_aux_def(self, aux, op, src):
         _chk(lib().opss_add_aux_def(self._h, int(aux), C.byref(_op(op)), int(src)))
+
+    def set_frame(self, field, axis, lo_width, lo_value, hi_width, hi_value):
+        _chk(lib().opss_set_frame(self._h, int(field), int(axis), int(lo_width), float(lo_value), int(hi_width), float(hi_value)))
 
     def add_aux_lhs(self, aux, op):
         _chk(lib().opss_add_aux_lhs(self._h, int(aux), C.byref(_op(op))))

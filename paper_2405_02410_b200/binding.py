@@ -18,7 +18,7 @@ F32, F64 = 0, 1
 DEALIAS_PAPER, DEALIAS_TWO_THIRDS, DEALIAS_OFF = 0, 1, 2
 OK, EINVAL, EUNSUPPORTED, ESTATE, ECUDA = 0, -1, -2, -3, -4
 
-SYMBOLS = ["pss_create", "pss_add_field", "pss_add_linear", "pss_add_aux_def", "pss_add_aux_lhs", "pss_add_aux_term", "pss_add_term",
+SYMBOLS = ["pss_create", "pss_add_field", "pss_add_linear", "pss_add_aux_def", "pss_add_aux_lhs", "pss_set_frame", "pss_add_aux_term", "pss_add_term",
            "pss_set_noise", "pss_set_dealias", "pss_set_replicas", "pss_select_replica", "pss_replicas", "pss_finalize", "pss_bind", "pss_set_field", "pss_step",
            "pss_get_field", "pss_get_field_fourier", "pss_set_field_fourier", "pss_set_step_count", "pss_debug_noise", "pss_profile_step", "pss_uses_fused_kernel", "pss_launch_count",
            "pss_model_bytes_per_step", "pss_step_count", "pss_strerror", "pss_last_cuda_error",
@@ -57,6 +57,7 @@ def lib():
         L.pss_add_field.argtypes = [P, C.c_char_p, C.c_int, C.POINTER(C.c_int)]
         L.pss_add_linear.argtypes = [P, C.c_int, C.POINTER(_Op)]
         L.pss_add_aux_def.argtypes = [P, C.c_int, C.POINTER(_Op), C.c_int]
+        L.pss_set_frame.argtypes = [P, C.c_int, C.c_int, C.c_int64, C.c_double, C.c_int64, C.c_double]
         L.pss_add_aux_lhs.argtypes = [P, C.c_int, C.POINTER(_Op)]
         L.pss_add_aux_term.argtypes = [P, C.c_int, C.POINTER(_Op), C.c_int, C.POINTER(C.c_int)]
         L.pss_add_term.argtypes = [P, C.c_int, C.POINTER(_Op), C.c_int, C.POINTER(C.c_int)]
@@ -152,6 +153,9 @@ class System:
 
     def add_aux_def(self, aux, op, src):
         self._chk(lib().pss_add_aux_def(self._h, int(aux), C.byref(_op(op)), int(src)))
+
+    def set_frame(self, field, axis, lo_width, lo_value, hi_width, hi_value):
+        self._chk(lib().pss_set_frame(self._h, int(field), int(axis), int(lo_width), float(lo_value), int(hi_width), float(hi_value)))
 
     def add_aux_lhs(self, aux, op):
         self._chk(lib().pss_add_aux_lhs(self._h, int(aux), C.byref(_op(op))))

@@ -24,12 +24,14 @@ namespace {
 
 struct DefH { pss_op op; int src; };
 struct ATermH { pss_op outer; std::vector<int> factors; };
+struct FrameH { int axis; long long lo_w, hi_w; double lo_v, hi_v; };
 struct FieldH {
   std::string name;
   bool dynamic;
   std::vector<DefH> defs;
   std::vector<pss_op> lhs;    /* dynamic: implicit terms; intermediate: its own lhs */
   std::vector<ATermH> aterms; /* intermediate: rhs terms that are products          */
+  std::vector<FrameH> frames; /* dynamic: Dirichlet buffer zones set at the end of every step */
   bool noisy;
   double D;
   int qpow;
@@ -969,7 +971,7 @@ int launch_fused(pss_system *s, int64_t nsteps) {
   return PSS_OK;
 }
 
-template <typename T> int do_steps(pss_system *s, int64_t nsteps) {
+template <typename T> int do_steps_core(pss_system *s, int64_t nsteps) {
   const Program &P = s->P;
   if (nsteps == 0) return PSS_OK;
   if (s->ndim == 1) {
@@ -1080,6 +1082,46 @@ template <typename T> int do_get_field(pss_system *s, int slot, void *dst, int o
   if (!on_device) {
     CK(cudaMemcpyAsync(dst, s->ws + s->off_ureal, (size_t)s->N * sizeof(T), cudaMemcpyDeviceToHost, s->stream));
     CK(cudaStreamSynchronize(s->stream));
+  }
+  return PSS_OK;
+}
+
+/* Dirichlet frames: the callback at the end of a time step.  The field goes to real space through the
+ * set/get kernels (device buffers only), the frame values are written, and it comes back; the next step then starts
+ * from the rebuilt factor arrays (prologue launch).  Functionality first: this costs a handful of extra launches per step. */
+template <typename T> __global__ void k_apply_frame(T *real, int nx, int ny, int nz, int axis, long long lo_w, long long hi_w, T lo_v, T hi_v) {
+  const size_t N = (size_t)nx * ny * nz;
+  const int na = axis == 0 ? nx : (axis == 1 ? ny : nz);
+  for (size_t x = (size_t)blockIdx.x * blockDim.x + threadIdx.x; x < N; x += (size_t)gridDim.x * blockDim.x) {
+    const long long c = axis == 0 ? (long long)(x % nx) : (axis == 1 ? (long long)((x / nx) % ny) : (long long)(x / ((size_t)nx * ny)));
+    if (c < lo_w) real[x] = lo_v;
+    else if (c >= na - hi_w) real[x] = hi_v;
+  }
+}
+
+template <typename T> int do_steps(pss_system *s, int64_t nsteps) {
+  bool any = false;
+  for (const FieldH &F : s->fields) if (!F.frames.empty()) any = true;
+  if (!any) return do_steps_core<T>(s, nsteps);
+  T *ureal = reinterpret_cast<T *>(s->ws + s->off_ureal);
+  const int sel0 = s->sel;
+  for (int64_t i = 0; i < nsteps; ++i) {
+    int rc = do_steps_core<T>(s, 1);
+    if (rc != PSS_OK) return rc;
+    for (int r = 0; r < s->nrep; ++r) {
+      s->sel = r;
+      for (size_t f = 0; f < s->fields.size(); ++f) {
+        const FieldH &F = s->fields[f];
+        if (F.frames.empty()) continue;
+        if ((rc = do_get_field<T>(s, s->dyn_slot[f], ureal, 1)) != PSS_OK) { s->sel = sel0; return rc; }
+        for (const FrameH &fr : F.frames) {
+          k_apply_frame<T><<<592, 256, 0, s->stream>>>(ureal, (int)s->n[0], (int)s->n[1], (int)s->n[2], fr.axis, fr.lo_w, fr.hi_w, (T)fr.lo_v, (T)fr.hi_v);
+          CKL("k_apply_frame");
+        }
+        if ((rc = do_set_field<T>(s, s->dyn_slot[f], ureal, 1)) != PSS_OK) { s->sel = sel0; return rc; }
+      }
+    }
+    s->sel = sel0;
   }
   return PSS_OK;
 }
@@ -1199,6 +1241,18 @@ int pss_add_aux_def(pss_system *s, int aux, const pss_op *op, int src) {
   if (!s->fields[src].dynamic && src >= aux) return PSS_EINVAL; /* A12 */
   DefH d; d.op = *op; d.src = src;
   s->fields[aux].defs.push_back(d);
+  return PSS_OK;
+}
+
+int pss_set_frame(pss_system *s, int field, int axis, int64_t lo_width, double lo_value, int64_t hi_width, double hi_value) {
+  if (!s) return PSS_EINVAL;
+  if (s->finalized) return PSS_ESTATE;
+  if (!fid_ok(s, field) || !s->fields[field].dynamic) return PSS_EINVAL;
+  if (axis < 0 || axis >= s->ndim) return PSS_EINVAL;
+  if (lo_width < 0 || hi_width < 0 || lo_width + hi_width > s->n[axis]) return PSS_EINVAL;
+  if (!std::isfinite(lo_value) || !std::isfinite(hi_value)) return PSS_EINVAL;
+  FrameH fr; fr.axis = axis; fr.lo_w = lo_width; fr.hi_w = hi_width; fr.lo_v = lo_value; fr.hi_v = hi_value;
+  s->fields[field].frames.push_back(fr);
   return PSS_OK;
 }
 

@@ -708,3 +708,57 @@ def test_p16_two_level_product_is_the_nested_direct_convolution(oracle, n):
                         acc += muh[k] * full[l] / n
             q2 = (2 * np.pi * q / n) ** 2
             assert abs(got[q] - (-q2) * acc) <= 1e-11 * max(1.0, abs(acc)), (dealias, q)
+
+
+# ------------------------------------------------------------------------------------------ P17
+def test_p17_dirichlet_frame_reaches_the_linear_steady_state(oracle):
+    """PAPER.md:233-255 and Fig. 2: heat diffusion dT/dt = d2T/dx2 between two baths on 256 sites, T(x,0) = 5.  With the
+    baths applied in a frame of width 10 (T(x < 10) = 10, T(x >= 246) = 0, set at the end of every step) the numerical
+    steady state is the analytical straight line between the baths; with the baths on single sites the periodic
+    representation leaves the artifact the paper shows (the profile stays far from the line)."""
+    n, dt, steps = 256, 2.0, 20000
+    x = np.arange(n)
+    err = {}
+    for w in (1, 10):
+        s = oracle.System((n,), (1.0,), dt, prec="f64", seed=1)
+        s.set_threads(1)
+        f = s.add_field("T", True)
+        s.add_linear(f, {"coef": 1.0, "q2_pow": 1})
+        s.set_frame(f, 0, w, 10.0, w, 0.0)
+        s.finalize()
+        s.set_field(f, np.full(n, 5.0))
+        s.step(steps)
+        T = s.get_field(f)
+        assert np.all(np.abs(T[:w] - 10.0) < 1e-12) and np.all(np.abs(T[n - w:]) < 1e-12)
+        lo, hi = w - 1, n - w
+        line = 10.0 * (hi - x) / (hi - lo)                    # T1 + (T2 - T1) x / L between the baths (PAPER.md:239)
+        sel = (x >= lo) & (x <= hi)
+        err[w] = np.abs(T - line)[sel].max()
+    assert err[10] < 0.01 * 10.0
+    assert err[1] > 0.2 * 10.0
+
+
+def test_p17_frame_semantics_2d(oracle):
+    """the frame is applied after Eq. 18, per axis, in the order given; elsewhere the field is what the step made it"""
+    n, dt = (16, 8), 0.1
+    rng = np.random.default_rng(17)
+    phi0 = rng.standard_normal(n[::-1])
+    a = oracle.System(n, (1.0, 1.0), dt, prec="f64", seed=5)
+    fa = a.add_field("phi", True)
+    a.add_linear(fa, {"coef": 1.0, "q2_pow": 1})
+    a.finalize()
+    b = oracle.System(n, (1.0, 1.0), dt, prec="f64", seed=5)
+    fb = b.add_field("phi", True)
+    b.add_linear(fb, {"coef": 1.0, "q2_pow": 1})
+    b.set_frame(fb, 0, 2, 1.5, 3, -2.0)
+    b.set_frame(fb, 1, 1, 7.0, 0, 0.0)
+    b.finalize()
+    a.set_field(fa, phi0)
+    b.set_field(fb, phi0)
+    a.step(1)
+    b.step(1)
+    want = a.get_field(fa).copy()
+    want[:, :2] = 1.5
+    want[:, 13:] = -2.0
+    want[:1, :] = 7.0
+    assert np.abs(b.get_field(fb) - want).max() < 1e-13
