@@ -135,10 +135,11 @@ int pss_set_step_count(pss_system *, uint64_t step);
 int pss_debug_noise(pss_system *, int field, uint64_t step, uint32_t *bits4_per_mode, void *z_halfspectrum);
 /* measurement hook: nsteps (<= 4096) steps exactly as pss_step, with one CUDA-event pair around every
  * kernel launch on the bound stream; synchronises.  Returns the mean device time per launch in ms and
- * the launch count of each kernel family: [0] k_rows, [1] k_update, [2] k_mid (3D only), [3] k_fused2d
- * (the persistent 1024^2 fp32 kernel: ONE launch runs all nsteps steps).  Not for 1D. */
+ * the launch count of each kernel family: [0] k_rows, [1] k_update, [2] k_mid (3D only), [3] the persistent 1024^2 fp32
+ * kernel (ONE launch runs all nsteps steps; which one: pss_uses_fused_kernel).  Not for 1D. */
 int pss_profile_step(pss_system *, int64_t nsteps, double ms_per_launch[4], int64_t launches[4]);
-/* 1 if this (finalized and bound) system steps with the persistent fused kernel, else 0. */
+/* 0: this (finalized and bound) system steps with the two generic kernels; 1: with the persistent kernel of
+ * pss_fused2d.cuh (f2d::k_fused2d / k_fused2d_pair); 2: with its second generation, pss_persist2d.cuh (p2d::k_persist2d). */
 int pss_uses_fused_kernel(const pss_system *);
 /* number of kernels this handle has launched so far (for bench.py's gpu_launches claim). */
 uint64_t pss_launch_count(const pss_system *);

@@ -268,6 +268,11 @@ class System:
     def uses_fused_kernel(self):
         return bool(lib().pss_uses_fused_kernel(self._h))
 
+    @property
+    def fused_kernel_name(self):
+        """None, or the persistent kernel that runs the steps"""
+        return {0: None, 1: "k_fused2d", 2: "k_persist2d"}[int(lib().pss_uses_fused_kernel(self._h))]
+
     def synchronize(self):
         self._torch_stream.synchronize()
 

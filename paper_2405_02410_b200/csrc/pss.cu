@@ -1494,7 +1494,10 @@ int pss_profile_step(pss_system *s, int64_t nsteps, double ms_per_launch[4], int
 
 uint64_t pss_launch_count(const pss_system *s) { return s ? s->launches : 0; }
 
-int pss_uses_fused_kernel(const pss_system *s) { return (s && s->finalized && s->bound && s->plan.fused) ? 1 : 0; }
+int pss_uses_fused_kernel(const pss_system *s) {
+  if (!(s && s->finalized && s->bound && s->plan.fused)) return 0;
+  return (s->plan.persist && s->nrep == 1) ? 2 : 1;
+}
 
 double pss_model_bytes_per_step(const pss_system *s, int pruned) {
   if (!s || !s->finalized) return 0.0;
