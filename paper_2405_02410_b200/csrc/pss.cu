@@ -736,7 +736,7 @@ int setup_fused(pss_system *s) {
     CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, f2d::k_fused2d<false>, f2d::THREADS, f2d::SMEM_BYTES));
   if (!coop || (long long)occ * nsm < f2d::NCTA) s->plan.fused = 0;
   s->plan.persist = 0;
-  if (s->plan.fused && s->plan.fused_prune && s->nrep == 1 && env_int("PSS_PERSIST", 1) != 0) {
+  if (s->plan.fused && s->plan.fused_prune && env_int("PSS_PERSIST", 1) != 0) {
     int occ3 = 0;
     CK(cudaFuncSetAttribute(p2d::k_persist2d, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p2d::SMEM_BYTES));
     CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ3, p2d::k_persist2d, p2d::THREADS, p2d::SMEM_BYTES));
@@ -898,7 +898,8 @@ int launch_fused(pss_system *s, int64_t nsteps) {
   /* an ensemble runs its replicas two per launch (k_fused2d_pair overlaps one replica's L2 exchanges with the
    * other's transforms), a last odd one alone; replica r: arrays [r], seed + r */
   for (int r = 0; r < s->nrep;) {
-    const bool pair = s->plan.fused_pair && r + 1 < s->nrep;
+    /* (the second-generation kernel runs the replicas one launch each: as fast per replica-step as the pair kernel) */
+    const bool pair = s->plan.fused_pair && !s->plan.persist && r + 1 < s->nrep;
     Program Pr = s->P;
     const uint64_t sd = s->seed + (uint64_t)r;
     Pr.seed_lo = (uint32_t)(sd & 0xffffffffu);
@@ -1496,7 +1497,7 @@ uint64_t pss_launch_count(const pss_system *s) { return s ? s->launches : 0; }
 
 int pss_uses_fused_kernel(const pss_system *s) {
   if (!(s && s->finalized && s->bound && s->plan.fused)) return 0;
-  return (s->plan.persist && s->nrep == 1) ? 2 : 1;
+  return s->plan.persist ? 2 : 1;
 }
 
 double pss_model_bytes_per_step(const pss_system *s, int pruned) {
