@@ -926,7 +926,7 @@ int launch_fused(pss_system *s, int64_t nsteps) {
       pa.tw = a.tw;
       pa.bar = a.bar + 32; /* 256 bytes past the first-generation counter; its two counters start from zero in every launch */
       pa.nsteps = nsteps; pa.step0 = s->step; pa.prologue = prologue;
-      pa.gate = env_int("PSS_NOISE_GATE", 1);
+      pa.gate = env_int("PSS_NOISE_GATE", 200);
       pa.prio = env_int("PSS_P2D_PRIO", 1);
       pa.dbg = env_int("PSS_P2D_DBG", 0);
       pa.ts = nullptr;
@@ -1353,6 +1353,10 @@ int pss_finalize(pss_system *s, size_t *workspace_bytes) {
   /* 3D: k_mid folds (array, replica) into gridDim.z (<= 65535) */
   if (s->ndim == 3 && (long long)(s->P.nfac > s->P.ngrp ? s->P.nfac : s->P.ngrp) * s->nrep > 65535) return PSS_EUNSUPPORTED;
   carve_workspace(s);
+  if (env_int("PSS_DEBUG_PLAN", 0))
+    std::fprintf(stderr, "pss plan: rounds %d ndyn %d nfac %d ngrp %d nlin %d rad_ok %d | upd W %d thr %d smem %zu blocks %d | rows Wc %d thr %d smem %zu blocks %d | fused %d\n",
+                 s->nround, s->P.ndyn, s->nfac_max, s->ngrp_max, s->P.nlin, s->P.rad_ok, s->plan.upd_W, s->plan.upd_threads,
+                 s->plan.upd_smem, s->plan.upd_blocks, s->plan.row_Wc, s->plan.row_threads, s->plan.row_smem, s->plan.row_blocks, s->plan.fused);
   s->finalized = true;
   if (workspace_bytes) *workspace_bytes = s->ws_need;
   return PSS_OK;

@@ -72,7 +72,7 @@ struct Args {
   unsigned long long step0;
   int prologue;                  /* 1: E is stale (after pss_set_field): rebuild it from the state first */
   int prio;                      /* 1: in phase C group 1 waits for group 0's transforms (PSS_P2D_PRIO=0 disables) */
-  int gate;                      /* 1: the noise warps pause while their group computes (PSS_NOISE_GATE=0 disables) */
+  int gate;                      /* > 0: the noise warps pause while their group computes, polling every `gate` ns (PSS_NOISE_GATE=0 disables) */
   int dbg;                       /* timing experiments only (-DPSS_P2D_DEBUG): 1 = skip the transforms, 2 = skip the noise */
   long long *ts;                 /* timing experiments only (-DPSS_P2D_DEBUG): globaltimer stamps [cta][group][32] of the last-but-one step */
 };
@@ -296,7 +296,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_persist2d(const __grid_constant_
         for (int r = 0; r < 16; r += 2) {
           /* pause while the group's transform warps compute; they clear the flag when they wait (exchange in flight,
            * or z itself needed) */
-          if (A.gate) while (hold[g]) __nanosleep(200);
+          if (A.gate) while (hold[g]) __nanosleep(A.gate);
           zw[r * TT] = noise_mode(K, kx, kyb + 16 * (r & 3) + 256 * (r >> 2), selfc);
           zw[(r + 1) * TT] = noise_mode(K, kx, kyb + 16 * ((r + 1) & 3) + 256 * ((r + 1) >> 2), selfc);
         }
