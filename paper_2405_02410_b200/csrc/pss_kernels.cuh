@@ -416,17 +416,46 @@ template <int SGN, typename T> __global__ void __launch_bounds__(256) k_mid(cons
   const int nn = A.nn[blockIdx.z % A.nbatch]; /* blockIdx.z runs over [replica][array] */
   if (nn && nn * kx >= A.nx) return;
   C *base = A.arr + (size_t)blockIdx.z * A.M + (size_t)kx * ny * A.nz + (size_t)blockIdx.x * W;
-  for (int idx = threadIdx.x; idx < ny * W; idx += blockDim.x) {
-    const int c = idx % W, j = idx / W;
+  const int lgW = 31 - __clz(W); /* W is a power of two (planner) */
+  if (sizeof(C) == 8 && W >= 2) {
+    /* fp32: two complex numbers per 16-byte access (W, nz and every offset above are even) */
+    const int lgH = lgW - 1;
+#pragma unroll 4
+    for (int idx = threadIdx.x; idx < (ny << lgH); idx += blockDim.x) {
+      const int c = (idx & ((W >> 1) - 1)) << 1, j = idx >> lgH;
+      int a = signed_index(j, ny);
+      a = a < 0 ? -a : a;
+      CPair<C> pr;
+      pr.a = pr.b = mk<C, T>((T)0, (T)0);
+      if (!(nn && nn * a >= ny)) pr = *reinterpret_cast<const CPair<C> *>(base + (size_t)j * A.nz + c);
+      C *d = sm + geo_pad(A.geo, j) * W + c;
+      d[0] = pr.a;
+      d[1] = pr.b;
+    }
+    __syncthreads();
+    fft_dif<SGN, T>(A.geo, sm, A.tw, W, W);
+#pragma unroll 4
+    for (int idx = threadIdx.x; idx < (ny << lgH); idx += blockDim.x) {
+      const int c = (idx & ((W >> 1) - 1)) << 1, s = idx >> lgH;
+      const C *q = sm + geo_pad(A.geo, s) * W + c;
+      CPair<C> pr;
+      pr.a = q[0];
+      pr.b = q[1];
+      *reinterpret_cast<CPair<C> *>(base + (size_t)geo_rev_fast(A.geo, s) * A.nz + c) = pr;
+    }
+    return;
+  }
+  for (int idx = threadIdx.x; idx < (ny << lgW); idx += blockDim.x) {
+    const int c = idx & (W - 1), j = idx >> lgW;
     int a = signed_index(j, ny);
     a = a < 0 ? -a : a;
     sm[geo_pad(A.geo, j) * W + c] = (nn && nn * a >= ny) ? mk<C, T>((T)0, (T)0) : base[(size_t)j * A.nz + c];
   }
   __syncthreads();
   fft_dif<SGN, T>(A.geo, sm, A.tw, W, W);
-  for (int idx = threadIdx.x; idx < ny * W; idx += blockDim.x) {
-    const int c = idx % W, s = idx / W;
-    base[(size_t)geo_rev(A.geo, s) * A.nz + c] = sm[geo_pad(A.geo, s) * W + c];
+  for (int idx = threadIdx.x; idx < (ny << lgW); idx += blockDim.x) {
+    const int c = idx & (W - 1), s = idx >> lgW;
+    base[(size_t)geo_rev_fast(A.geo, s) * A.nz + c] = sm[geo_pad(A.geo, s) * W + c];
   }
 }
 
