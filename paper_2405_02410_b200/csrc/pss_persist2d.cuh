@@ -2,8 +2,8 @@
  * pss_persist2d.cuh — the whole time step of a 1024 x 1024 fp32 single-field system with a cubic
  * (cutoff <= N/4) de-aliasing mask as ONE persistent cooperative kernel, second generation.
  *
- * What changed against pss_fused2d.cuh (which stays for the other de-aliasing rules and for replica pairs).  The
- * timeline of that kernel (globaltimer stamps, profiles/r2_persist2d.md) showed half of the step in the two all-to-all
+ * What changed against pss_fused2d.cuh (which stays for the other de-aliasing rules).  The
+ * timeline of that kernel (globaltimer stamps, profiles/r2_summary.md) showed half of the step in the two all-to-all
  * exchanges, and its per-thread 8-byte global accesses touching 4-8 different 128-byte lines per warp instruction.
  * Here
  *   - each exchange array is laid out per CONSUMER CTA as one contiguous block made of 128-byte chunks, one chunk per
@@ -17,7 +17,11 @@
  *     the third of the instructions that is noise goes where the issue slots are free;
  *   - a CTA's 256 transform threads are two independent 128-thread groups (2 lines each) with their own named
  *     barriers, so one group's exchange traffic overlaps the other's transforms; group 0 owns the two de-aliased
- *     (kept) columns, whose inverse transform feeds the next exchange, group 1 the two columns outside the mask.
+ *     (kept) columns, whose inverse transform feeds the next exchange, and runs first in phase C; group 1 owns the two
+ *     columns outside the mask (no inverse transform): it arrives at barrier B with a relaxed reduction as soon as its
+ *     input block is fetched and transforms while that barrier is in flight.
+ * Bulk asynchronous copies (cp.async.bulk + mbarrier) and two flag-in-data protocols without a grid barrier were built
+ * and measured for these exchanges and were not faster (profiles/r2_summary.md).
  *
  * Transform.  1024 = 16 x 16 x 4, three register passes around two shared-memory exchanges (as pss_fused2d.cuh):
  *   natural n = 64 n1 + 4 n2 + n3, spectral k = k1 + 16 k2 + 256 k3
