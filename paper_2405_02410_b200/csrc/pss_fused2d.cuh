@@ -185,12 +185,17 @@ __device__ __forceinline__ void grid_barrier(unsigned long long *ctr, unsigned l
   tsync();
   if ((threadIdx.x & (TT - 1)) == 0) {
     asm volatile("red.release.gpu.global.add.u64 [%0], 1;" ::"l"(ctr) : "memory");
-    unsigned long long v;
+    unsigned long long v, t0 = 0;
     unsigned spins = 0;
     for (;;) {
       asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(ctr) : "memory");
       if (v >= target) break;
-      if (++spins > (1u << 25)) __trap(); /* watchdog (tens of seconds): fail the launch instead of hanging the GPU */
+      if (((++spins) & 0x3fffu) == 0) { /* watchdog on the wall clock (30 s): fail the launch instead of hanging the GPU */
+        unsigned long long t;
+        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+        if (t0 == 0) t0 = t;
+        else if (t - t0 > 30000000000ull) __trap();
+      }
     }
   }
   tsync();
