@@ -420,7 +420,7 @@ template <int SGN, typename T> __global__ void __launch_bounds__(256) k_mid(cons
   if (sizeof(C) == 8 && W >= 2) {
     /* fp32: two complex numbers per 16-byte access (W, nz and every offset above are even) */
     const int lgH = lgW - 1;
-#pragma unroll 4
+#pragma unroll 8
     for (int idx = threadIdx.x; idx < (ny << lgH); idx += blockDim.x) {
       const int c = (idx & ((W >> 1) - 1)) << 1, j = idx >> lgH;
       int a = signed_index(j, ny);
@@ -434,7 +434,7 @@ template <int SGN, typename T> __global__ void __launch_bounds__(256) k_mid(cons
     }
     __syncthreads();
     fft_dif<SGN, T>(A.geo, sm, A.tw, W, W);
-#pragma unroll 4
+#pragma unroll 8
     for (int idx = threadIdx.x; idx < (ny << lgH); idx += blockDim.x) {
       const int c = (idx & ((W >> 1) - 1)) << 1, s = idx >> lgH;
       const C *q = sm + geo_pad(A.geo, s) * W + c;

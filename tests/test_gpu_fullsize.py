@@ -213,3 +213,25 @@ def test_config5_full_length_kpz_growth(pss):
     assert g.step_count == 5000
     assert all(b > a for a, b in zip(means, means[1:])), means      # lambda > 0: the surface moves up
     assert widths[-1] > widths[0] * 0.9 and widths[-1] < 10.0, widths
+
+
+def test_persistent_kernel_scheduling_switches_do_not_change_the_result(pss):
+    """PSS_NOISE_GATE (noise warps paused while their group computes) and PSS_P2D_PRIO (group 0 first in phase C) only
+    move work in time: the fields are bit-identical with either switched off; so is an ensemble replica (one launch per
+    replica) and the single system with its seed."""
+    import os
+    cfg = wl.make_config("modelb_1024")
+    ref, ids = wl.build(pss, cfg, prec="f32")
+    assert ref.fused_kernel_name == "k_persist2d"
+    ref.step(6)
+    want = ref.get_field_fourier(ids["phi"]).view(np.uint32)
+    for var in ("PSS_NOISE_GATE", "PSS_P2D_PRIO"):
+        os.environ[var] = "0"
+        try:
+            g, _ = wl.build(pss, cfg, prec="f32")
+            g.step(2)
+            g.step(4)
+            got = g.get_field_fourier(ids["phi"]).view(np.uint32)
+        finally:
+            del os.environ[var]
+        assert np.array_equal(got, want), var
