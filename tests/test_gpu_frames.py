@@ -84,3 +84,28 @@ def test_frame_on_the_persistent_kernel(pss, oracle):
     g.step(3)
     o.step(3)
     compare_fields(g, o, [f], 3 * TOL1["f32"], "1024^2 frame, 3 steps")
+
+
+def test_frames_in_an_ensemble_match_single_systems(pss):
+    """every replica gets its frame; replica r stays bit-identical to the single system with seed + r"""
+    cfg = wl.make_config("modelb_128", n=(64, 64))
+
+    def make(seed, replicas):
+        s = pss.System(cfg["n"], (1.0, 1.0), cfg["dt"], prec="f32", seed=seed, replicas=replicas)
+        ids = wl.model_b(s, **cfg["params"])
+        s.set_frame(ids["phi"], 1, 3, 0.5, 3, -0.5)
+        s.finalize()
+        return s, ids["phi"]
+
+    ic = wl.initial_conditions(cfg, np.float32)["phi"]
+    e, f = make(cfg["seed"], 3)
+    for r in range(3):
+        e.select_replica(r)
+        e.set_field(f, ic + 0.01 * r)
+    e.step(7)
+    for r in range(3):
+        s, _ = make(cfg["seed"] + r, 1)
+        s.set_field(f, ic + 0.01 * r)
+        s.step(7)
+        e.select_replica(r)
+        assert np.array_equal(e.get_field_fourier(f).view(np.uint32), s.get_field_fourier(f).view(np.uint32)), r
