@@ -184,11 +184,14 @@ def make_config(name, n=None, **over):
     return cfg
 
 
-def initial_conditions(cfg, dtype=np.float64):
-    """{field name: array shaped n[::-1]} from the config's seed (A16)."""
+def initial_conditions(cfg, dtype=np.float64, ids=None):
+    """{field name: array shaped n[::-1]} from the config's seed (A16).  The Philox counter carries the field id:
+    ``ids[name]`` when the caller has them (``build``), else the position in ``cfg["ic"]`` (the same number for every
+    workload here, whose dynamic fields are created first)."""
     shape = tuple(cfg["n"])[::-1]
     out = {}
-    for fid, (name, rng) in enumerate(cfg["ic"].items()):
+    for pos, (name, rng) in enumerate(cfg["ic"].items()):
+        fid = pos if ids is None else ids[name]
         if rng is None:
             out[name] = np.zeros(shape, dtype=dtype)
         else:
@@ -212,6 +215,6 @@ def build(api, cfg, prec="f32", dealias=None, set_ic=True, **sys_kwargs):
     s.finalize()
     if set_ic:
         dtype = np.float32 if prec == "f32" else np.float64
-        for name, arr in initial_conditions(cfg, dtype).items():
+        for name, arr in initial_conditions(cfg, dtype, ids).items():
             s.set_field(ids[name], arr)
     return s, ids
