@@ -1506,19 +1506,24 @@ int pss_uses_fused_kernel(const pss_system *s) {
 
 double pss_model_bytes_per_step(const pss_system *s, int pruned) {
   if (!s || !s->finalized) return 0.0;
-  const Program &P = s->P;
   const double S = (double)s->N * (double)s->rsize * (double)s->nrep;
-  if (s->ndim == 1) return 2.0 * P.ndyn * S;
-  double c1 = 0.0, c2 = 0.0; /* sum over factors of the kept fraction per axis, and its square */
-  for (int f = 0; f < P.nfac; ++f) {
-    double c = 1.0;
-    if (pruned && P.dealias != PSS_DEALIAS_OFF)
-      c = 2.0 / (double)((P.dealias == PSS_DEALIAS_TWO_THIRDS ? 2 : P.fac[f].order) + 1);
-    c1 += c;
-    c2 += c * c;
+  if (s->ndim == 1) return 2.0 * s->P.ndyn * S;
+  /* every spectral source is read and written once per step; every round (one per dependency level of the
+   * product-defined intermediate fields, the dynamic equations last) moves its groups and the kept band of its factors */
+  double total = 2.0 * s->P.ndyn * S;
+  for (const Program &P : s->PR) {
+    double c1 = 0.0, c2 = 0.0; /* sum over factors of the kept fraction per axis, and its square */
+    for (int f = 0; f < P.nfac; ++f) {
+      double c = 1.0;
+      if (pruned && P.dealias != PSS_DEALIAS_OFF)
+        c = 2.0 / (double)((P.dealias == PSS_DEALIAS_TWO_THIRDS ? 2 : P.fac[f].order) + 1);
+      c1 += c;
+      c2 += c * c;
+    }
+    if (s->ndim == 2) total += S * (2.0 * P.ngrp + 2.0 * c1);
+    else total += S * (4.0 * P.ngrp + 2.0 * c2 + 2.0 * c1);
   }
-  if (s->ndim == 2) return S * (2.0 * P.ndyn + 2.0 * P.ngrp + 2.0 * c1);
-  return S * (2.0 * P.ndyn + 4.0 * P.ngrp + 2.0 * c2 + 2.0 * c1);
+  return total;
 }
 
 uint64_t pss_step_count(const pss_system *s) { return s ? s->step : 0; }
