@@ -381,6 +381,9 @@ def kernel_bytes(cfg, S, g, steps_per_fused_launch):
     # update : ngrp (read) + 2 ndyn + sum_f c_f^(ndim-1) (write)
     table = {"model_b": (1, 1, [0.5]), "kpz": (1, 1, [2 / 3.0] * ndim),
              "nematic": (2, 2, [0.5, 0.5] + [2 / 3.0] * 7), "diffusion": (1, 0, [])}
+    if model not in table:  # several rounds of the two kernels (product-defined intermediate fields): no per-kernel split
+        nl = {"k_rows": 3, "k_update": 3}
+        return {"k_rows": total / 2 / nl["k_rows"], "k_update": total / 2 / nl["k_update"], "k_mid": 0.0, "k_fused2d": total * steps_per_fused_launch}
     ndyn, ngrp, cs = table[model]
     rows = S * (sum(cs) + ngrp)
     upd = S * (ngrp + 2 * ndyn + sum(c ** (ndim - 1) for c in cs))

@@ -146,6 +146,34 @@ def nematic(s, A=-1.0, C=1.0, K=1.0, lam=1.0, alpha=-2.0, eta=1.0, D=1e-3):
             "Exx": exx, "Exy": exy}
 
 
+def model_h(s, k=1.0, eta=2.0, D=0.005):
+    """Binary fluid ("model H" class) in stream-function form, stated through the equation-string
+    front end: chemical potential mu = phi^3 - phi + k q^2 phi (a product-defined intermediate field), Stokes flow driven
+    by the capillary force, eta q^4 w = d_x mu d_y phi - d_y mu d_x phi (an intermediate field with its own lhs),
+    v = (d_y w, -d_x w), dt phi = -q^2 mu - v.grad phi with the stiff part implicit.  The paper's own Model H listing is
+    not in the paper; this is a model of the same structure (several intermediate fields, two dependency levels)."""
+    from .equations import Model
+    m = Model(s)
+    m.add_parameter("k", k)
+    m.add_parameter("eta", eta)
+    m.add_parameter("D", D)
+    m.create_field("phi", True)
+    for name in ("mu", "dxphi", "dyphi", "dxmu", "dymu", "w", "vx", "vy"):
+        m.create_field(name, False)
+    m.add_equation("mu = phi^3 - phi + k*q^2*phi")
+    m.add_equation("dxphi = iqx*phi")
+    m.add_equation("dyphi = iqy*phi")
+    m.add_equation("dxmu = iqx*mu")
+    m.add_equation("dymu = iqy*mu")
+    m.add_equation("eta*q^4*w = dxmu*dyphi - dymu*dxphi")
+    m.add_equation("vx = iqy*w")
+    m.add_equation("vy = -iqx*w")
+    m.add_equation("dt phi + k*q^4*phi = -q^2*phi^3 + q^2*phi - vx*dxphi - vy*dyphi")
+    if D > 0:
+        m.add_noise("phi", "D*q^2")
+    return m.ids()
+
+
 # --------------------------------------------------------------------------------------------
 # BASELINE.json configs (seeds: DESIGN.md "Input recipe")
 # --------------------------------------------------------------------------------------------
@@ -167,7 +195,11 @@ for _e in range(8, 14):  # Model-B lattice sweep 256^2 .. 8192^2 (config-2 equat
     CONFIGS["sweep_%d" % _n] = dict(model="model_b", n=(_n, _n), dx=1.0, dt=0.01, steps=1000, seed=2405024106,
                                     params=dict(a=-1.0, b=1.0, k=1.0, D=0.05), ic={"phi": (0.05, 0.15)})
 
-MODELS = {"model_b": model_b, "kpz": kpz, "nematic": nematic, "diffusion": diffusion}
+# not a BASELINE config: the multi-round path on the lattice of the headline
+CONFIGS["modelh_1024"] = dict(model="model_h", n=(1024, 1024), dx=1.0, dt=0.005, steps=1000, seed=2405024108,
+                              params=dict(k=1.0, eta=2.0, D=0.005), ic={"phi": (-0.1, 0.1)})
+
+MODELS = {"model_b": model_b, "kpz": kpz, "nematic": nematic, "diffusion": diffusion, "model_h": model_h}
 
 
 def make_config(name, n=None, **over):

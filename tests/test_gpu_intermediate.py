@@ -142,3 +142,17 @@ def test_unsupported_combinations(pss):
     with pytest.raises(b.PssError) as e:
         s.finalize(bind=False)
     assert e.value.code == b.EUNSUPPORTED
+
+
+def test_model_h_workload_at_1024_squared(pss, oracle):
+    """the `modelh_1024` workload bench.py can time (three rounds of the step kernels per time step), full size"""
+    cfg = wl.make_config("modelh_1024")
+    g, ids = wl.build(pss, cfg, prec="f32")
+    o, _ = wl.build(oracle, cfg, prec="f32")
+    g.step(1)
+    o.step(1)
+    compare_fields(g, o, [ids["phi"]], TOL1["f32"], "modelh_1024 1 step")
+    g.step(9)
+    o.step(9)
+    compare_fields(g, o, [ids["phi"]], 10 * TOL1["f32"], "modelh_1024 10 steps")
+    assert not g.uses_fused_kernel
