@@ -2,11 +2,11 @@
 
 Two metrics per dynamic field, both CUDA path vs. oracle on the same seeded inputs:
   * relative L2 over the real-space field (north_star's tolerance, PAPER.md:125 iterated), and
-  * a per-mode check on the half-spectrum: max_q |phi_q(gpu) - phi_q(oracle)| / (rms + |phi_q(oracle)|), rms = the
-    rms magnitude of the q != 0 modes (a mode much larger than the rest, e.g. the mean, is measured against itself).  An L2 over 10^6..10^8 sites can dilute one wrong boundary-plane or Nyquist mode at the long
-    horizons (one mode of typical size that is entirely wrong has ratio ~1); rounding errors are spread over all
-    modes, so their maximum over M modes stays within a few sigma of the L2 figure.  The bound is
-    MODE_FACTOR x the L2 tolerance, applied against the rms of the fluctuating (q != 0) part of the spectrum.
+  * a per-mode check on the half-spectrum: max_q |phi_q(gpu) - phi_q(oracle)| / (rms + |phi_q(oracle)|), rms = the rms
+    magnitude of the q != 0 modes (a mode much larger than the rest, e.g. the mean, is measured against itself).  An
+    L2 over 10^6..10^8 sites can dilute one wrong boundary-plane or Nyquist mode at the long horizons (one mode of
+    typical size that is entirely wrong has ratio ~0.5); rounding errors are spread over all modes, so their maximum
+    over M modes stays within a few sigma of the L2 figure.  The bound is MODE_FACTOR x the L2 tolerance.
 """
 import numpy as np
 
