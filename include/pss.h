@@ -21,7 +21,8 @@
  *
  * Ownership: the caller owns every buffer it passes and must keep the bound workspace alive until
  * pss_destroy (or the next pss_bind).  The library owns the opaque handle and small host tables.
- * Handles are not thread-safe.  No exceptions cross this boundary; there is no global state.
+ * Handles are not thread-safe.  No exceptions cross this boundary; there is no global state apart from the fixed device
+ * array behind pss_debug_noise_noalloc (described there).
  *
  * Errors: every int-returning call gives 0 on success or a negative code:
  *   PSS_EINVAL        bad id / negative power / NULL / aux used before defined / implicit term on aux
@@ -30,6 +31,7 @@
  *                     table capacities exceeded (see PSS_MAX_*)
  *   PSS_ESTATE        add_* after finalize; bind/step/get before finalize/bind
  *   PSS_ECUDA         a CUDA call failed (sticky for the handle; text via pss_last_cuda_error)
+ *   PSS_ETOOBIG       pss_debug_noise_noalloc only: the lattice has more than PSS_STATIC_NOISE_MAX_MODES modes
  */
 #ifndef PSS_H
 #define PSS_H
@@ -43,7 +45,7 @@ typedef struct pss_system pss_system;
 
 typedef enum { PSS_F32 = 0, PSS_F64 = 1 } pss_precision;
 enum { PSS_DEALIAS_PAPER = 0, PSS_DEALIAS_TWO_THIRDS = 1, PSS_DEALIAS_OFF = 2 };
-enum { PSS_OK = 0, PSS_EINVAL = -1, PSS_EUNSUPPORTED = -2, PSS_ESTATE = -3, PSS_ECUDA = -4 };
+enum { PSS_OK = 0, PSS_EINVAL = -1, PSS_EUNSUPPORTED = -2, PSS_ESTATE = -3, PSS_ECUDA = -4, PSS_ETOOBIG = -5 };
 
 /* capacities of the device-side term program */
 enum {
@@ -133,6 +135,35 @@ int pss_set_step_count(pss_system *, uint64_t step);
 /* test hook for the noise stream (HOST pointers, either may be NULL): the 4 Philox4x32-10 words per
  * logical mode m, and the unit Hermitian Gaussian z (complex of the system precision) the step uses. */
 int pss_debug_noise(pss_system *, int field, uint64_t step, uint32_t *bits4_per_mode, void *z_halfspectrum);
+/* pss_debug_noise without any allocation.  Same arguments, same kernel, same values (bit for bit); the only difference
+ * is where the kernel's results wait on the device before they are copied to `bits4_per_mode` / `z_halfspectrum`.
+ *
+ * Why it exists.  pss_debug_noise is the one call of this library that asks the CUDA runtime for device memory
+ * (cudaMalloc, released with cudaFree before it returns).  A program built around this library often cannot afford
+ * that, or is not allowed to:
+ *   - the usual host is a PyTorch (or RMM, or other pooling) process whose caching allocator already holds nearly
+ *     all of the GPU's memory; a raw cudaMalloc then fails with "out of memory" although the pool has plenty free;
+ *   - cudaFree waits for ALL work on the device, so checking the noise stream from a monitoring thread stalls every
+ *     other stream of a running simulation or training job;
+ *   - while any thread of the process is capturing a CUDA graph in the default (global) capture mode, cudaMalloc is
+ *     an illegal call: it fails and breaks that thread's capture.
+ * Such callers use this entry point: it calls no cudaMalloc, cudaFree or any library routine that allocates.
+ *
+ * How.  The staging area is a fixed array compiled into the library, PSS_STATIC_NOISE_MAX_MODES * 32 bytes
+ * (16.03 MiB: room for the 1024 x 513 half-spectrum of the headline lattice in either precision).  The CUDA runtime
+ * places it on every GPU on which the library is loaded and keeps it there until the process exits, whether or not
+ * this call is ever made.  A system with more modes (n0/2+1)*n1*n2 than that gets PSS_ETOOBIG and nothing is launched.
+ *
+ * First call on a device: it looks up the array's device address (cudaGetSymbolAddress) and keeps it for later
+ * calls.  Make that first call at set-up time, before any stream capture begins.
+ *
+ * Sharing: there is ONE array per GPU for the whole process.  Every call overwrites what the previous one left there
+ * (each call writes all it later reads, so stale contents never reach the caller and nothing needs clearing).  A call
+ * returns only after its results are in host memory, but two calls that are in flight at the same time on one GPU —
+ * from two threads, through two handles or streams — write the same bytes and corrupt each other: serialise them.
+ * HOST pointers, either may be NULL, as for pss_debug_noise. */
+enum { PSS_STATIC_NOISE_MAX_MODES = 1024 * 513 };
+int pss_debug_noise_noalloc(pss_system *, int field, uint64_t step, uint32_t *bits4_per_mode, void *z_halfspectrum);
 /* measurement hook: nsteps (<= 4096) steps exactly as pss_step, with one CUDA-event pair around every
  * kernel launch on the bound stream; synchronises.  Returns the mean device time per launch in ms and
  * the launch count of each kernel family: [0] k_rows, [1] k_update, [2] k_mid (3D only), [3] the persistent 1024^2 fp32

@@ -16,11 +16,12 @@ from . import build as _build
 
 F32, F64 = 0, 1
 DEALIAS_PAPER, DEALIAS_TWO_THIRDS, DEALIAS_OFF = 0, 1, 2
-OK, EINVAL, EUNSUPPORTED, ESTATE, ECUDA = 0, -1, -2, -3, -4
+OK, EINVAL, EUNSUPPORTED, ESTATE, ECUDA, ETOOBIG = 0, -1, -2, -3, -4, -5
+STATIC_NOISE_MAX_MODES = 1024 * 513   # include/pss.h: capacity of the fixed device array behind debug_noise_noalloc
 
 SYMBOLS = ["pss_create", "pss_add_field", "pss_add_linear", "pss_add_aux_def", "pss_add_aux_lhs", "pss_set_frame", "pss_add_aux_term", "pss_add_term",
            "pss_set_noise", "pss_set_dealias", "pss_set_replicas", "pss_select_replica", "pss_replicas", "pss_finalize", "pss_bind", "pss_set_field", "pss_step",
-           "pss_get_field", "pss_get_field_fourier", "pss_set_field_fourier", "pss_set_step_count", "pss_debug_noise", "pss_profile_step", "pss_uses_fused_kernel", "pss_launch_count",
+           "pss_get_field", "pss_get_field_fourier", "pss_set_field_fourier", "pss_set_step_count", "pss_debug_noise", "pss_debug_noise_noalloc", "pss_profile_step", "pss_uses_fused_kernel", "pss_launch_count",
            "pss_model_bytes_per_step", "pss_step_count", "pss_strerror", "pss_last_cuda_error",
            "pss_destroy"]
 
@@ -75,6 +76,7 @@ def lib():
         L.pss_set_field_fourier.argtypes = [P, C.c_int, P, C.c_int]
         L.pss_set_step_count.argtypes = [P, C.c_uint64]
         L.pss_debug_noise.argtypes = [P, C.c_int, C.c_uint64, P, P]
+        L.pss_debug_noise_noalloc.argtypes = [P, C.c_int, C.c_uint64, P, P]
         L.pss_profile_step.argtypes = [P, C.c_int64, C.POINTER(C.c_double), C.POINTER(C.c_int64)]
         L.pss_uses_fused_kernel.argtypes = [P]
         L.pss_launch_count.argtypes = [P]
@@ -255,6 +257,20 @@ class System:
         z = np.empty(self.hshape, dtype=self.cdtype)
         self._chk(lib().pss_debug_noise(self._h, int(field), C.c_uint64(int(step)),
                                         bits.ctypes.data_as(C.c_void_p), z.ctypes.data_as(C.c_void_p)))
+        return bits.reshape(self.hshape + (4,)), z
+
+    def debug_noise_noalloc(self, field, step):
+        """``debug_noise`` for processes that must not, or cannot, call cudaMalloc/cudaFree (a framework's memory pool
+        owns the GPU, a device-wide synchronisation is unaffordable, or a graph capture is under way elsewhere in the
+        process): pss_debug_noise_noalloc stages the values in a fixed 16 MiB device array that is part of libpss.so.
+        Same values as ``debug_noise``.  At most STATIC_NOISE_MAX_MODES modes (PssError ETOOBIG beyond); one array per
+        GPU, so do not run two of these calls at the same time on one GPU.  Make the first call on each GPU at set-up
+        time, before any stream capture."""
+        nm = int(np.prod(self.hshape))
+        bits = np.empty((nm, 4), dtype=np.uint32)
+        z = np.empty(self.hshape, dtype=self.cdtype)
+        self._chk(lib().pss_debug_noise_noalloc(self._h, int(field), C.c_uint64(int(step)),
+                                                bits.ctypes.data_as(C.c_void_p), z.ctypes.data_as(C.c_void_p)))
         return bits.reshape(self.hshape + (4,)), z
 
     def profile_step(self, n):

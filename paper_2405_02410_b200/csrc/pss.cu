@@ -13,6 +13,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <string>
 #include <vector>
 
@@ -1171,6 +1172,53 @@ template <typename T> int do_debug_noise(pss_system *s, int field, uint64_t step
   return PSS_OK;
 }
 
+/* ---- the one entry point that allocates nothing: pss_debug_noise_noalloc --------------------------------------------
+ * pss_debug_noise stages its device-side results in two buffers it gets from cudaMalloc and gives back with cudaFree.
+ * Here the same kernel writes into a fixed array that is part of the library image instead.  The array is sized for the
+ * half-spectrum of the headline lattice (1024 x 513 modes: 16 bytes of Philox words plus at most 16 bytes of z each,
+ * 16.03 MiB); every GPU on which the library gets loaded carries it until the process exits, used or not. */
+constexpr size_t STATIC_NOISE_BYTES = (size_t)PSS_STATIC_NOISE_MAX_MODES * 32;
+static __device__ __align__(256) unsigned char g_static_noise[STATIC_NOISE_BYTES];
+
+/* `g_static_noise` in HOST code is only a handle the runtime knows the symbol by, not an address a kernel could use, so
+ * the device address is asked for once per device (with that device current) and remembered.  The table is per process;
+ * the mutex only serialises the look-up, not the use of the array. */
+constexpr int STATIC_MAX_DEVICES = 64;
+std::mutex g_static_mu;
+void *g_static_ptr[STATIC_MAX_DEVICES] = {};
+
+int static_noise_ptr(pss_system *s, unsigned char **out) {
+  int dev = -1;
+  CK(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= STATIC_MAX_DEVICES) return PSS_EUNSUPPORTED;
+  std::lock_guard<std::mutex> lk(g_static_mu);
+  if (!g_static_ptr[dev]) {
+    void *p = nullptr;
+    CK(cudaGetSymbolAddress(&p, g_static_noise));
+    if (!p) return cuda_fail(s, cudaErrorInvalidSymbol, "cudaGetSymbolAddress(g_static_noise)");
+    g_static_ptr[dev] = p;
+  }
+  *out = (unsigned char *)g_static_ptr[dev];
+  return PSS_OK;
+}
+
+template <typename T> int do_debug_noise_noalloc(pss_system *s, int field, uint64_t step, uint32_t *bits, void *z) {
+  typedef typename cplx_of<T>::type C;
+  unsigned char *base = nullptr;
+  const int rc = static_noise_ptr(s, &base);
+  if (rc != PSS_OK) return rc;
+  /* words first, z behind them at the capacity offset (a multiple of 256 bytes); the kernel writes every element the
+   * copies below read, so nothing left behind by an earlier call is ever seen and nothing needs clearing */
+  uint32_t *dbits = bits ? reinterpret_cast<uint32_t *>(base) : nullptr;
+  C *dz = z ? reinterpret_cast<C *>(base + (size_t)PSS_STATIC_NOISE_MAX_MODES * 16) : nullptr;
+  k_debug_noise<T><<<592, 256, 0, s->stream>>>(s->P, (unsigned)s->sel, field, step, dbits, dz);
+  CKL("k_debug_noise");
+  if (bits) CK(cudaMemcpyAsync(bits, dbits, (size_t)s->M * 4 * sizeof(uint32_t), cudaMemcpyDeviceToHost, s->stream));
+  if (z) CK(cudaMemcpyAsync(z, dz, (size_t)s->M * sizeof(C), cudaMemcpyDeviceToHost, s->stream));
+  CK(cudaStreamSynchronize(s->stream));
+  return PSS_OK;
+}
+
 }  // namespace
 
 /* ---- C ABI ----------------------------------------------------------------------------- */
@@ -1458,6 +1506,17 @@ int pss_debug_noise(pss_system *s, int field, uint64_t step, uint32_t *bits, voi
                               : do_debug_noise<double>(s, field, step, bits, z);
 }
 
+int pss_debug_noise_noalloc(pss_system *s, int field, uint64_t step, uint32_t *bits, void *z) {
+  if (!s) return PSS_EINVAL;
+  if (!s->finalized || !s->bound) return PSS_ESTATE;
+  if (s->cuda_bad) return PSS_ECUDA;
+  if (s->M > (int64_t)PSS_STATIC_NOISE_MAX_MODES) return PSS_ETOOBIG;
+  DeviceGuard guard(s->dev);
+  if (!fid_ok(s, field)) return PSS_EINVAL;
+  return (s->prec == PSS_F32) ? do_debug_noise_noalloc<float>(s, field, step, bits, z)
+                              : do_debug_noise_noalloc<double>(s, field, step, bits, z);
+}
+
 int pss_profile_step(pss_system *s, int64_t nsteps, double ms_per_launch[4], int64_t launches[4]) {
   if (!s || nsteps < 0 || nsteps > 4096 || !ms_per_launch || !launches) return PSS_EINVAL;
   if (!s->finalized || !s->bound) return PSS_ESTATE;
@@ -1535,6 +1594,7 @@ const char *pss_strerror(int code) {
     case PSS_EUNSUPPORTED: return "unsupported configuration";
     case PSS_ESTATE: return "call made in the wrong state";
     case PSS_ECUDA: return "CUDA error (see pss_last_cuda_error)";
+    case PSS_ETOOBIG: return "lattice has more modes than the library's fixed device array holds (PSS_STATIC_NOISE_MAX_MODES)";
     default: return "unknown error";
   }
 }
