@@ -5,7 +5,7 @@
     python bench.py --impl reference ...            # the CPU oracle, timed on the host cores
 
 One bench "step" is one call pss_step(inner): `inner` consecutive time steps of the whole hot path
-(k_rows + k_update per time step, or all of them inside one persistent k_fused2d launch at 1024^2 fp32) on the workload's lattice.  The state of a time stepper is consumed by
+(k_rows + k_update per time step, or all of them inside one persistent p2d::k_persist2d launch at 1024^2 fp32) on the workload's lattice.  The state of a time stepper is consumed by
 the next time step, so inside one bench step the working set is as warm as the workload makes it; BETWEEN
 timed bench steps L2 is flushed (a 256 MiB buffer is written), so every timed step starts cold.
 

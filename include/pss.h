@@ -103,7 +103,7 @@ int pss_set_dealias(pss_system *, int rule);
  * `nreplicas` independent realisations of the same field system and pss_step advances all of them in the same
  * launches (grid dimension y).  Replica r is, bit for bit, the system created with seed + r.  Call before
  * pss_finalize; 1 <= nreplicas <= 65535, and in 3D additionally max(#factor fields, #product groups) * nreplicas
- * <= 65535 (pss_finalize returns PSS_EUNSUPPORTED otherwise).  The persistent 2D kernel runs the replicas two per launch. */
+ * <= 65535 (pss_finalize returns PSS_EUNSUPPORTED otherwise).  The persistent 1024^2 kernel (p2d::k_persist2d) runs one launch per replica. */
 int pss_set_replicas(pss_system *, int nreplicas);
 /* which replica pss_set_field / pss_get_field / pss_get_field_fourier / pss_debug_noise address (default 0) */
 int pss_select_replica(pss_system *, int replica);

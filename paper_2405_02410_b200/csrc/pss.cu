@@ -50,7 +50,7 @@ struct Plan {
   int fused_prune;                  /* its input-pruned instantiation (mask cutoff <= n/4 on both axes)       */
   int pdl;                          /* programmatic dependent launch between the step kernels (PSS_PDL=0 disables) */
   int fused_pair;                   /* ensembles: two replicas per launch (k_fused2d_pair)                    */
-  int persist;                      /* 1: pss_persist2d.cuh's kernel (cutoff <= N/4: bulk-copy exchanges) runs single systems (PSS_PERSIST=0 disables) */
+  int persist;                      /* 1: pss_persist2d.cuh's kernel (cutoff <= N/4; cp.async.cg block fetches behind two grid-barrier counters) runs the steps, one launch per replica (PSS_PERSIST=0 disables) */
 };
 
 }  // namespace
@@ -896,8 +896,9 @@ int launch_fused(pss_system *s, int64_t nsteps) {
   const int prologue = s->psix_valid ? 0 : 1;
   const void *fn1 = s->plan.fused_prune ? (const void *)f2d::k_fused2d<true> : (const void *)f2d::k_fused2d<false>;
   const void *fn2 = s->plan.fused_prune ? (const void *)f2d::k_fused2d_pair<true> : (const void *)f2d::k_fused2d_pair<false>;
-  /* an ensemble runs its replicas two per launch (k_fused2d_pair overlaps one replica's L2 exchanges with the
-   * other's transforms), a last odd one alone; replica r: arrays [r], seed + r */
+  /* replica r: arrays [r], seed + r.  With the second-generation kernel (plan.persist, the default rule) every replica
+   * gets its own launch; only the first-generation fallback pairs them (k_fused2d_pair overlaps one replica's L2
+   * exchanges with the other's transforms, a last odd one alone) */
   for (int r = 0; r < s->nrep;) {
     /* (the second-generation kernel runs the replicas one launch each: as fast per replica-step as the pair kernel) */
     const bool pair = s->plan.fused_pair && !s->plan.persist && r + 1 < s->nrep;
@@ -919,7 +920,8 @@ int launch_fused(pss_system *s, int64_t nsteps) {
     void *params[2] = {(void *)&Pr, (void *)&a};
     cudaError_t e;
     if (!pair && s->plan.persist) {
-      /* second-generation kernel (pss_persist2d.cuh): flag-in-data exchanges, no barrier counters */
+      /* second-generation kernel (pss_persist2d.cuh): two grid-barrier counters (bar[0], bar[16]; zeroed before every launch),
+       * exchange blocks fetched with cp.async.cg; an ensemble gets one launch per replica */
       p2d::Args pa;
       pa.state = a.state;
       pa.Eg = a.E; /* the factor array and the group array hold the two exchange arrays */
