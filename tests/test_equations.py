@@ -169,3 +169,36 @@ def test_parsed_and_hand_written_systems_give_the_same_trajectory(oracle):
     a.step(20)
     s.step(20)
     assert np.array_equal(a.get_field(ids["phi"]), s.get_field(m.ids()["phi"]))
+
+
+def _readme_python_blocks():
+    import os
+    import re
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    return re.findall(r"```python\n(.*?)```", open(os.path.join(root, "README.md")).read(), flags=re.S)
+
+
+def test_readme_equation_example_is_stable(oracle):
+    """The front-page equation-string example, run as printed (the oracle's System standing in for the GPU one): the
+    stiff k*q^4 term must sit on the implicit side (reading A8 makes anything on the rhs explicit; with k = 4, dt = 0.01,
+    dx = 1 an explicit k*q^4 has an Euler factor of about -14 at the top mode), so 100 steps from a noisy start stay
+    finite and bounded."""
+    blocks = [b for b in _readme_python_blocks() if "add_equation" in b]
+    assert len(blocks) == 1
+    src = blocks[0]
+    assert "pss.System(" in src and "dt phi + k*q^4*phi" in src
+
+    class _Shim:                                   # `pss.System` of the snippet -> the CPU oracle, smaller lattice
+        @staticmethod
+        def System(n, dx, dt, **kw):
+            return oracle.System((64, 64), dx, dt, **kw)
+
+    env = {"pss": _Shim}
+    exec(compile(src, "README.md", "exec"), env)
+    s, phi = env["s"], env["phi"]
+    rng = np.random.default_rng(7)
+    s.set_field(phi, (0.1 * rng.standard_normal((64, 64))).astype(np.float32))
+    s.step(100)
+    x = np.asarray(s.get_field(phi), dtype=np.float64)
+    assert np.isfinite(x).all()
+    assert np.max(np.abs(x)) < 2.0                 # frames are +-1, the bulk stays inside the double well
