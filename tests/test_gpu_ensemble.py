@@ -34,6 +34,8 @@ def test_replicas_equal_single_systems_and_oracle(pss, oracle, name, n):
     dyn_names = list(cfg["ic"].keys())
     ens, ids = wl.build(pss, cfg, prec="f32", set_ic=False, replicas=R)
     assert ens.replicas == R
+    if n == (1024, 1024):   # the one-launch-per-replica path of the persistent kernel (seed + r, counters cleared per launch)
+        assert ens.fused_kernel_name == "k_persist2d"
     for r in range(R):
         cr = dict(cfg, seed=cfg["seed"] + r)
         ens.select_replica(r)
@@ -45,7 +47,7 @@ def test_replicas_equal_single_systems_and_oracle(pss, oracle, name, n):
     for r in range(R):
         cr = dict(cfg, seed=cfg["seed"] + r)
         one, _ = wl.build(pss, cr, prec="f32")
-        assert one.uses_fused_kernel == ens.uses_fused_kernel
+        assert one.fused_kernel_name == ens.fused_kernel_name
         one.step(steps)
         o, _ = wl.build(oracle, cr, prec="f32")
         o.step(steps)

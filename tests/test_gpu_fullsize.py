@@ -217,8 +217,9 @@ def test_config5_full_length_kpz_growth(pss):
 
 def test_persistent_kernel_scheduling_switches_do_not_change_the_result(pss):
     """PSS_NOISE_GATE (noise warps paused while their group computes) and PSS_P2D_PRIO (group 0 first in phase C) only
-    move work in time: the fields are bit-identical with either switched off; so is an ensemble replica (one launch per
-    replica) and the single system with its seed."""
+    move work in time: the fields are bit-identical with either switched off.  (That an ensemble replica, one k_persist2d
+    launch per replica, is bit-identical to the single system with its seed is checked at 1024^2 in
+    test_gpu_ensemble.py::test_replicas_equal_single_systems_and_oracle.)"""
     import os
     cfg = wl.make_config("modelb_1024")
     ref, ids = wl.build(pss, cfg, prec="f32")
