@@ -173,6 +173,8 @@ def main():
                     help="ensemble: R independent realisations stepped in the same launches (value counts replica-steps)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-compare", action="store_true", help="skip the cuFFT+cuRAND comparison step (2D Model B only)")
+    ap.add_argument("--no-secondary", action="store_true",
+                    help="skip the short timed legs of the other BASELINE configs that the default (headline) run appends under `secondary`")
     args = ap.parse_args()
 
     rank = int(os.environ.get("RANK", "0"))
@@ -299,7 +301,10 @@ def main():
         dom_ms = prof[dom][0]
         dom_name = (g.fused_kernel_name or dom) if dom == "k_fused2d" else dom   # which persistent kernel ran
         P = g  # algorithmic bytes per launch of each kernel family
-        kb = kernel_bytes(cfg, S * R, g, prof_n)
+        # the persistent kernel's launches are cut at the Hermitian-projection period (pss.cu HERM_PERIOD) and run one
+        # replica each: time steps one launch advances = prof_n * R / launches
+        fused_steps = prof_n * R / max(1, prof["k_fused2d"][1])
+        kb = kernel_bytes(cfg, S * R, g, fused_steps / R)
         ach = kb[dom] / (dom_ms * 1e-3) / 1e9
         line = {
             "metric": "timesteps/s", "value": value, "unit": "timesteps/s", "n_gpus": world, "steps": args.steps,
@@ -317,7 +322,7 @@ def main():
                          "frac": ach / peak, "traffic": (ncu_traffic(args.workload, dom_name) or {}).get("dram_bytes_per_launch"),
                          "traffic_capture": ncu_traffic(args.workload, dom_name), "peak_source": peak_src,
                          "algorithmic_bytes_per_launch": kb[dom], "launch_ms": dom_ms,
-                         "timesteps_per_launch": prof_n if dom == "k_fused2d" else 1,
+                         "timesteps_per_launch": fused_steps if dom == "k_fused2d" else 1,
                          "kernel_ms": {(dom_name if k == dom else k): v[0] for k, v in prof.items() if v[1] > 0},
                          "kernel_share": {(dom_name if k == dom else k): shares[k] / sum(shares.values()) for k in shares}},
             "roofline_step": {"B_alg_bytes": b_alg, "B_model_bytes": b_model,
@@ -333,19 +338,72 @@ def main():
             nsm = torch.cuda.get_device_properties(dev).multi_processor_count
             mhz = (clocks or {}).get("sm_mhz") or 1965.0
             wi_step = R * tr["warp_instr_per_launch"] / tr["timesteps_per_launch"]  # the capture ran one replica
-            t_dom = dom_ms * 1e-3 / (prof_n if dom == "k_fused2d" else 1)
+            t_dom = dom_ms * 1e-3 * (prof["k_fused2d"][1] / prof_n if dom == "k_fused2d" else 1)   # dominant kernel's time per time step
             line["roofline"]["issue"] = {"bound": "alu", "unit": "warp-instr/s", "achieved": wi_step / t_dom,
                                          "peak": 4.0 * nsm * mhz * 1e6, "frac": wi_step / t_dom / (4.0 * nsm * mhz * 1e6),
                                          "note": "instruction-issue slots: 4 schedulers per SM x 1 warp-instr per clock"}
+            # `frac` above is BASELINE.json's target metric: ALGORITHMIC bytes against the HBM peak.  What the kernel really
+            # pulls from DRAM (the committed ncu capture) can be far less when the working set stays in L2: say so, and name
+            # the resource that is actually closest to its ceiling.
+            dram_step = R * tr["dram_bytes_per_launch"] / tr["timesteps_per_launch"]
+            dram_frac = dram_step / t_dom / 1e9 / peak
+            line["roofline"]["frac_meaning"] = "algorithmic bytes per launch / launch time / measured HBM peak (BASELINE.json target metric)"
+            line["roofline"]["dram_frac_measured"] = dram_frac
+            line["roofline"]["limiter"] = ("issue slots / L2 round trips (working set L2-resident: measured DRAM traffic is %.1f%% of the algorithmic bytes)"
+                                           % (100.0 * dram_step / b_alg)
+                                           if line["roofline"]["issue"]["frac"] > dram_frac else "hbm")
         if not args.no_cpu_baseline and world == 1:
             r, n, el, cores = oracle_rate(cfg, args.prec, args.cpu_budget, 10 ** 6)
             line["cpu_baseline"] = {"value": r, "unit": "timesteps/s", "cores": cores, "kind": "oracle",
                                     "sample": "%d oracle time steps of %s after 1 warm-up step, %.1f s" % (n, args.workload, el)}
         if not args.no_compare and world == 1 and cfg["model"] == "model_b" and len(cfg["n"]) == 2 and args.prec == "f32":
             line["cufft_curand_comparison"] = cufft_compare(cfg)
+        if not args.no_secondary and world == 1 and R == 1 and args.workload == "modelb_1024" and args.prec == "f32":
+            del g
+            line["secondary"] = secondary_legs(pss, torch, dev, stream, flush, peak)
         print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
+
+
+SECONDARY = ("sweep_4096", "kpz_4096", "modelb_256c", "nematic_1024", "modelb_128")
+
+
+def secondary_legs(pss, torch, dev, stream, flush, peak):
+    """Short timed legs of the other BASELINE.json configs, so that the driver's own run clocks more than the headline:
+    per workload 3 warm-up calls and 3 timed calls of pss_step(20) (60 timed time steps), CUDA events on the launching
+    stream, L2 flushed before every timed call, state resident in HBM; fp32, one replica, no oracle leg.
+    frac_alg = B_alg (pss_model_bytes_per_step, pruned) / time per time step / measured HBM peak."""
+    out = {}
+    for name in SECONDARY:
+        try:
+            c = wl.make_config(name)
+            s, ids = wl.build(pss, c, prec="f32", device=str(dev))
+            inner, calls = 20, 3
+            for _ in range(3):
+                s.step(inner)
+            if c["model"] == "nematic":   # A20: the literal parameters blow up after ~400 steps; 60 + 60 stay well inside
+                for nm, arr in wl.initial_conditions(c, s.rdtype).items():
+                    s.set_field(ids[nm], arr)
+                s.step(inner)
+            torch.cuda.synchronize(dev)
+            ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(calls)]
+            for i in range(calls):
+                flush.fill_(i + 1)
+                ev[i][0].record(stream)
+                s.step(inner)
+                ev[i][1].record(stream)
+            torch.cuda.synchronize(dev)
+            us = 1e3 * sum(a.elapsed_time(b) for a, b in ev) / (calls * inner)
+            b_alg = s.model_bytes_per_step(True)
+            fin = bool(np.isfinite(s.get_field(ids[list(c["ic"].keys())[0]])).all())
+            out[name] = {"us_per_timestep": us, "frac_alg": b_alg / (us * 1e-6) / 1e9 / peak, "B_alg_bytes": b_alg,
+                         "lattice": list(c["n"]), "timed_timesteps": calls * inner, "kernel": s.fused_kernel_name or "k_rows+k_update",
+                         "final_state_finite": fin}
+            del s
+        except Exception as e:  # a secondary leg never takes the headline line down with it
+            out[name] = {"unavailable": repr(e)[:200]}
+    return out
 
 
 def cufft_compare(cfg):

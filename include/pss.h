@@ -174,6 +174,13 @@ int pss_profile_step(pss_system *, int64_t nsteps, double ms_per_launch[4], int6
 int pss_uses_fused_kernel(const pss_system *);
 /* number of kernels this handle has launched so far (for bench.py's gpu_launches claim). */
 uint64_t pss_launch_count(const pss_system *);
+/* The state is kept in Fourier space for the whole run.  On the planes kx = 0 and kx = n0/2 the half-spectrum stores both
+ * members of each conjugate pair, and only their Hermitian combination belongs to the real field; the
+ * rest is rounding residue that Eq. 18 would amplify wherever L_q > 0.  pss_step therefore replaces those pairs by their
+ * Hermitian mean after every step whose number (pss_step_count) is a multiple of the period returned here (a power of
+ * two <= 1024 chosen at pss_finalize from the largest 1/|1 - dt L_q|; 0 before pss_finalize).  The schedule depends on
+ * the step number only, so splitting a run into several pss_step calls, or restoring a checkpoint, changes nothing. */
+int64_t pss_hermitian_period(const pss_system *);
 /* algorithmic bytes one step of this system must move: pruned != 0 gives B_alg,
  * pruned == 0 gives B_model. */
 double pss_model_bytes_per_step(const pss_system *, int pruned);

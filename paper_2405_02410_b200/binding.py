@@ -21,7 +21,7 @@ STATIC_NOISE_MAX_MODES = 1024 * 513   # include/pss.h: capacity of the fixed dev
 
 SYMBOLS = ["pss_create", "pss_add_field", "pss_add_linear", "pss_add_aux_def", "pss_add_aux_lhs", "pss_set_frame", "pss_add_aux_term", "pss_add_term",
            "pss_set_noise", "pss_set_dealias", "pss_set_replicas", "pss_select_replica", "pss_replicas", "pss_finalize", "pss_bind", "pss_set_field", "pss_step",
-           "pss_get_field", "pss_get_field_fourier", "pss_set_field_fourier", "pss_set_step_count", "pss_debug_noise", "pss_debug_noise_noalloc", "pss_profile_step", "pss_uses_fused_kernel", "pss_launch_count",
+           "pss_get_field", "pss_get_field_fourier", "pss_set_field_fourier", "pss_set_step_count", "pss_debug_noise", "pss_debug_noise_noalloc", "pss_profile_step", "pss_uses_fused_kernel", "pss_launch_count", "pss_hermitian_period",
            "pss_model_bytes_per_step", "pss_step_count", "pss_strerror", "pss_last_cuda_error",
            "pss_destroy"]
 
@@ -80,6 +80,8 @@ def lib():
         L.pss_profile_step.argtypes = [P, C.c_int64, C.POINTER(C.c_double), C.POINTER(C.c_int64)]
         L.pss_uses_fused_kernel.argtypes = [P]
         L.pss_launch_count.argtypes = [P]
+        L.pss_hermitian_period.argtypes = [P]
+        L.pss_hermitian_period.restype = C.c_int64
         L.pss_launch_count.restype = C.c_uint64
         L.pss_model_bytes_per_step.argtypes = [P, C.c_int]
         L.pss_model_bytes_per_step.restype = C.c_double
@@ -295,6 +297,12 @@ class System:
     @property
     def step_count(self):
         return int(lib().pss_step_count(self._h))
+
+    @property
+    def hermitian_period(self):
+        """pss_step projects the planes kx = 0 and kx = n0/2 of the state onto Hermitian symmetry after every step whose
+        number is a multiple of this (include/pss.h, pss_hermitian_period)"""
+        return int(lib().pss_hermitian_period(self._h))
 
     @property
     def launch_count(self):

@@ -66,6 +66,7 @@ struct pss_system {
   int nrep, sel; /* ensemble: replicas of the same field system (replica r = seed + r), selected replica for set/get */
   bool finalized, bound, psix_valid;
   uint64_t step;
+  int64_t herm_period; /* the state is projected onto Hermitian symmetry whenever step % herm_period == 0 (plan_hermitian) */
   std::vector<FieldH> fields;
   std::vector<TermH> terms;
   std::vector<int> dyn_slot; /* field -> spectral source slot (dynamic fields, then product-defined intermediate fields), else -1 */
@@ -975,7 +976,7 @@ int launch_fused(pss_system *s, int64_t nsteps) {
   return PSS_OK;
 }
 
-template <typename T> int do_steps_core(pss_system *s, int64_t nsteps) {
+template <typename T> int do_steps_chunk(pss_system *s, int64_t nsteps) {
   const Program &P = s->P;
   if (nsteps == 0) return PSS_OK;
   if (s->ndim == 1) {
@@ -1007,6 +1008,120 @@ template <typename T> int do_steps_core(pss_system *s, int64_t nsteps) {
       if ((rc = launch_update<T>(s, 0, s->step, s->PU[(size_t)k])) != PSS_OK) return rc;
     }
     s->step += 1;
+  }
+  return PSS_OK;
+}
+
+/* Hermitian projection of the state (reading A25).  The fields are real, so on the two planes of the
+ * half-spectrum that hold both members of a conjugate pair, kx = 0 and kx = nx/2, the state must satisfy
+ * phi(-k) = conj(phi(k)).  The state of this library lives in Fourier space for the whole run and is never rebuilt from
+ * real space, and rounding breaks that symmetry by one ulp per step.  The C2R transforms ignore the anti-Hermitian part,
+ * so the nonlinear terms never see it and cannot saturate it; Eq. 18 multiplies it by 1/(1 - dt L_q) every step like
+ * any other mode.  Where L_q > 0 (Model B's spinodal band, rate 1/4 per unit time at q^2 = 1/2) it grows without bound:
+ * measured at 1024^2 fp32, as large as the largest physical mode after 10^4 steps, NaN after 2 10^4.  Every
+ * herm_period-th step (counted on the absolute step number, so that pss_step(a); pss_step(b) == pss_step(a + b) and a
+ * restored checkpoint continue bit for bit) the pairs are replaced by their Hermitian mean and the self-conjugate modes
+ * lose their imaginary part: the identity in exact arithmetic, idempotent in floating point.  The factor arrays are
+ * rebuilt from the projected state (prologue), again so that a run restored from a checkpoint taken there agrees. */
+/* The period.  Between two projections the anti-Hermitian part may grow by at most a factor 16: with
+ * g = max over the two planes and the dynamic fields of |1/(1 - dt L_q)| (evaluated on the host in double),
+ * period = largest power of two <= ln 16 / ln g.  That analysis is complete for a single dynamic field without explicit
+ * linear terms (nothing else acts on the anti-Hermitian part): cap 1024.  Explicit linear terms couple the fields'
+ * anti-Hermitian parts in ways the diagonal factor does not bound: cap 128 there.  Model B, dt = 0.01: g = 1.0025, 1024. */
+int64_t plan_hermitian(const pss_system *s) {
+  const double two_pi = 6.283185307179586476925286766559;
+  bool simple = true;
+  int ndynf = 0;
+  for (const FieldH &F : s->fields) ndynf += F.dynamic ? 1 : 0;
+  for (const TermH &t : s->terms) if (t.factors.size() == 1) simple = false;
+  if (ndynf != 1) simple = false;
+  const int64_t cap = simple ? 1024 : 128;
+  double lng = 0.0;
+  for (const FieldH &F : s->fields) {
+    if (!F.dynamic || F.lhs.empty()) continue;
+    for (int hi = 0; hi < 2; ++hi)
+      for (int64_t k2 = 0; k2 < s->n[2]; ++k2)
+        for (int64_t k1 = 0; k1 < s->n[1]; ++k1) {
+          const int64_t kk[3] = {hi ? s->n[0] / 2 : 0, k1, k2};
+          double q[3] = {0, 0, 0}, q2 = 0.0;
+          bool nyq[3] = {false, false, false};
+          for (int j = 0; j < s->ndim; ++j) {
+            const int64_t sk = (2 * kk[j] <= s->n[j]) ? kk[j] : kk[j] - s->n[j];
+            q[j] = two_pi * (double)sk / ((double)s->n[j] * s->dx[j]);
+            nyq[j] = s->n[j] > 1 && 2 * kk[j] == s->n[j];
+            q2 += q[j] * q[j];
+          }
+          double lre = 0.0, lim = 0.0; /* L_q = -sum coef Op(q) (pss_add_linear) */
+          for (const pss_op &op : F.lhs) {
+            double r = op.coef * std::pow(q2, op.q2_pow);
+            if (op.invq_pow > 0) r = (q2 > 0.0) ? r * std::pow(q2, -0.5 * op.invq_pow) : 0.0;
+            int sdeg = 0;
+            for (int j = 0; j < 3; ++j) {
+              if (op.iq_pow[j] > 0) r = (nyq[j] && (op.iq_pow[j] & 1)) ? 0.0 : r * std::pow(q[j], op.iq_pow[j]);
+              sdeg += op.iq_pow[j];
+            }
+            switch (sdeg & 3) { case 0: lre -= r; break; case 1: lim -= r; break; case 2: lre += r; break; default: lim += r; }
+          }
+          const double dre = 1.0 - s->dt * lre, dim = -s->dt * lim, d2 = dre * dre + dim * dim;
+          if (d2 < 1.0) lng = std::max(lng, d2 > 0.0 ? -0.5 * std::log(d2) : 1e300);
+        }
+  }
+  if (lng <= 0.0) return cap;
+  const double lim16 = std::log(16.0) / lng;
+  int64_t p = 1;
+  while (2 * p <= cap && (double)(2 * p) <= lim16) p *= 2;
+  return p;
+}
+
+template <typename T>
+__global__ void k_hermitize(typename cplx_of<T>::type *state, long long stride, int nxh, int ny, int nz) {
+  typedef typename cplx_of<T>::type C;
+  C *const arr = state + (size_t)blockIdx.y * (size_t)stride; /* internal layout: [kx][y][z] */
+  const long long plane = (long long)ny * nz;
+  for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < 2 * plane; i += (long long)gridDim.x * blockDim.x) {
+    const bool hi = i >= plane;
+    const long long idx = hi ? i - plane : i;
+    const int y = (int)(idx / nz), z = (int)(idx % nz);
+    const long long pidx = (long long)((ny - y) % ny) * nz + (nz - z) % nz;
+    if (idx > pidx) continue; /* the pair is handled by its lower index */
+    C *const p = arr + (hi ? (size_t)(nxh - 1) * (size_t)plane : (size_t)0);
+    C a = p[idx];
+    if (idx == pidx) {
+      a.y = (T)0;
+      p[idx] = a;
+    } else {
+      C b = p[pidx];
+      a.x = (T)0.5 * (a.x + b.x);
+      a.y = (T)0.5 * (a.y - b.y);
+      b.x = a.x;
+      b.y = -a.y;
+      p[idx] = a;
+      p[pidx] = b;
+    }
+  }
+}
+
+template <typename T> int launch_hermitize(pss_system *s) {
+  const long long plane = (long long)s->n[1] * s->n[2];
+  const unsigned bx = (unsigned)std::min<long long>(592, (2 * plane + 255) / 256);
+  const int narr = s->nrep * s->P.ndyn; /* state arrays: [replica][dynamic field], arr_stride apart */
+  for (int a0 = 0; a0 < narr; a0 += 65535) {
+    const int na = std::min(65535, narr - a0);
+    k_hermitize<T><<<dim3(bx, (unsigned)na), 256, 0, s->stream>>>(carr<T>(s, s->off_state, a0), arr_stride(s), s->P.nxh, (int)s->n[1], (int)s->n[2]);
+    CKL("k_hermitize");
+  }
+  s->psix_valid = false;
+  return PSS_OK;
+}
+
+/* nsteps steps, cut at the multiples of herm_period of the absolute step number */
+template <typename T> int do_steps_core(pss_system *s, int64_t nsteps) {
+  while (nsteps > 0) {
+    const int64_t n = std::min<int64_t>(nsteps, s->herm_period - (int64_t)(s->step % (uint64_t)s->herm_period));
+    int rc = do_steps_chunk<T>(s, n);
+    if (rc != PSS_OK) return rc;
+    nsteps -= n;
+    if (s->step % (uint64_t)s->herm_period == 0 && (rc = launch_hermitize<T>(s)) != PSS_OK) return rc;
   }
   return PSS_OK;
 }
@@ -1403,6 +1518,7 @@ int pss_finalize(pss_system *s, size_t *workspace_bytes) {
   /* 3D: k_mid folds (array, replica) into gridDim.z (<= 65535) */
   if (s->ndim == 3 && (long long)(s->P.nfac > s->P.ngrp ? s->P.nfac : s->P.ngrp) * s->nrep > 65535) return PSS_EUNSUPPORTED;
   carve_workspace(s);
+  s->herm_period = plan_hermitian(s);
   if (env_int("PSS_DEBUG_PLAN", 0))
     std::fprintf(stderr, "pss plan: rounds %d ndyn %d nfac %d ngrp %d nlin %d rad_ok %d | upd W %d thr %d smem %zu blocks %d | rows Wc %d thr %d smem %zu blocks %d | fused %d\n",
                  s->nround, s->P.ndyn, s->nfac_max, s->ngrp_max, s->P.nlin, s->P.rad_ok, s->plan.upd_W, s->plan.upd_threads,
@@ -1559,6 +1675,8 @@ int pss_profile_step(pss_system *s, int64_t nsteps, double ms_per_launch[4], int
 }
 
 uint64_t pss_launch_count(const pss_system *s) { return s ? s->launches : 0; }
+
+int64_t pss_hermitian_period(const pss_system *s) { return (s && s->finalized) ? s->herm_period : 0; }
 
 int pss_uses_fused_kernel(const pss_system *s) {
   if (!(s && s->finalized && s->bound && s->plan.fused)) return 0;
