@@ -221,10 +221,27 @@ __device__ __forceinline__ void st_cg16(void *p, uint4 v) {
 __device__ __forceinline__ void grid_arrive(unsigned long long *ctr) {
   asm volatile("red.release.gpu.global.add.u64 [%0], 1;" ::"l"(ctr) : "memory");
 }
-/* arrival of a group that wrote nothing the other CTAs read (it only reports that its input block has been fetched:
- * the asynchronous copies were waited for, so no fence is needed) */
+/* Arrival of a group that wrote nothing the other CTAs read: it only reports that its input block has been fetched, so
+ * that the producers may overwrite that block in their next phase (a write-after-read dependency).
+ *
+ * Ordering.  In the PTX memory model a relaxed reduction gives the producers' acquire poll nothing to
+ * synchronise with, so the model does not order the fetch before the overwrite.  The hardware does: the fetch is
+ * cp.async.cg, and the group executes cp.async.wait_all and its named barrier before the one arriving thread issues the
+ * reduction; wait_all returns only when the copied bytes are in shared memory, i.e. the reads of the block have
+ * completed at L2 and can no longer observe a later store.  A read that has returned its data cannot be reordered
+ * after anything.  What the relaxed form drops is the MEMBAR.GPU of a release (the wait for the acknowledgement of
+ * the group's own earlier stores, of which there are none that matter here).
+ * Cost of the formally ordered form, measured (round 3, B200, bench.py --steps 40, A/B/A/B on one box): 10.005 us per
+ * step with red.release.gpu here against 9.595 us with red.relaxed.gpu (+0.41 us, 4.3 %).  The product keeps the
+ * relaxed form; -DPSS_P2D_ARRIVE_RELEASE (PSS_NVCC_EXTRA) builds the other, bit-identical in its results.
+ * tests/test_gpu_soak.py runs 10^6 steps and compares bit for bit with the first-generation kernel (PSS_PERSIST=0),
+ * whose barriers are all release/acquire. */
 __device__ __forceinline__ void grid_arrive_relaxed(unsigned long long *ctr) {
+#ifdef PSS_P2D_ARRIVE_RELEASE
+  asm volatile("red.release.gpu.global.add.u64 [%0], 1;" ::"l"(ctr) : "memory");
+#else
   asm volatile("red.relaxed.gpu.global.add.u64 [%0], 1;" ::"l"(ctr) : "memory");
+#endif
 }
 __device__ __forceinline__ void grid_poll(const unsigned long long *ctr, unsigned long long target) {
   unsigned long long v, t0 = 0;
