@@ -251,6 +251,10 @@ def main():
     ms = [a.elapsed_time(b) for a, b in ev]
     total_ms = float(sum(ms))
     clocks = sampler.stop() if sampler else None
+    # the state the TIMED steps ended on (the e2e leg below reloads the initial condition, so its output says nothing
+    # about the long run)
+    g.select_replica(0)
+    timed_finite = all(bool(np.isfinite(g.get_field_fourier(ids[n_]).view(g.rdtype)).all()) for n_ in dyn_names)
 
     # ---- e2e: host buffers through the public API, copies inside the timed region ----
     host_in = [{name: torch.from_numpy(arr).pin_memory() for name, arr in ics[r].items()} for r in range(R)]
@@ -312,7 +316,7 @@ def main():
             "scaling": "weak", "vs_baseline": None, "dtype": args.prec, "data": "synthetic",
             "site_updates_per_s": value * sites, "us_per_timestep": step_ms * 1e3, "us_per_replica_timestep": step_ms * 1e3 / R,
             "config": bench_config(args, cfg, R),
-            "final_state_finite": finite,
+            "final_state_finite": bool(finite and timed_finite), "timed_state_finite": timed_finite,
             "gpu_launches": int(launches_timed),
             "clocks": clocks,
             "e2e": {"value": e2e_value, "unit": "timesteps/s",
