@@ -930,11 +930,12 @@ int launch_fused(pss_system *s, int64_t nsteps) {
       pa.tw = a.tw;
       pa.bar = a.bar + 32; /* 256 bytes past the first-generation counter; its two counters start from zero in every launch */
       pa.nsteps = nsteps; pa.step0 = s->step; pa.prologue = prologue;
-      pa.gate = env_int("PSS_NOISE_GATE", 200);
-      pa.prio = env_int("PSS_P2D_PRIO", 1);
-      pa.dbg = env_int("PSS_P2D_DBG", 0);
+      pa.gate = std::min(std::max(env_int("PSS_NOISE_GATE", 200), 0), 100000); /* poll interval in ns, 0 = gate off */
+      pa.prio = env_int("PSS_P2D_PRIO", 1) != 0 ? 1 : 0;
+      pa.dbg = 0; /* knock-out switches and time stamps exist in -DPSS_P2D_DEBUG builds only */
       pa.ts = nullptr;
 #ifdef PSS_P2D_DEBUG
+      pa.dbg = env_int("PSS_P2D_DBG", 0);
       pa.ts = env_int("PSS_P2D_TS", 0) ? reinterpret_cast<long long *>(s->ws + s->off_scratch) : nullptr;
 #endif
       CK(cudaMemsetAsync(pa.bar, 0, 256, s->stream));
